@@ -1,0 +1,35 @@
+"""Helpers for the oracle pin tests: simple hand-built cases (plain data)."""
+import numpy as np
+
+from paper_2412_04395_b200 import workloads as wl
+
+
+def uniform_case(nx, ny, nz, dx, dy, dz, theta0=300.0, rho0=1.0, g=0.0, **par):
+    """Uniform base state (no gravity unless asked), flat uniform grid."""
+    p = dict(wl.DEFAULT_PARAMS)
+    p.update(g=g)
+    p.update(par)
+    zl = np.arange(nz + 1, dtype=np.float64) * dz
+    return dict(name="uniform", nx=nx, ny=ny, nz=nz, dx=dx, dy=dy, z_nodes=None, z_levels=zl,
+                rho0=np.full(nz, rho0), rhotheta0=np.full(nz, rho0 * theta0), params=p)
+
+
+def zeros_state(case):
+    nx, ny, nz = case["nx"], case["ny"], case["nz"]
+    c = (nz, ny, nx)
+    return [np.zeros(c), np.zeros(c), np.zeros(c), np.zeros((nz + 1, ny, nx)), np.zeros(c)]
+
+
+def base_state_fields(case):
+    """(rho0, Theta0) broadcast to [nz][ny][nx]."""
+    nx, ny, nz = case["nx"], case["ny"], case["nz"]
+    r0, t0 = case["rho0"], case["rhotheta0"]
+    if r0.ndim == 1:
+        r0 = np.broadcast_to(r0[:, None, None], (nz, ny, nx))
+        t0 = np.broadcast_to(t0[:, None, None], (nz, ny, nx))
+    return np.array(r0), np.array(t0)
+
+
+def rel_err(a, b, scale=None):
+    s = scale if scale is not None else max(np.abs(b).max(), 1e-300)
+    return float(np.abs(a - b).max() / s)
