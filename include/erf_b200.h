@@ -1,0 +1,131 @@
+/*
+ * erf_b200.h -- C-ABI of liberf_b200.so: one RK3 step of the dry, compressible,
+ * non-hydrostatic dynamical core of ERF (arXiv 2412.04395) on one B200 (sm_100a).
+ *
+ * PAPER.md = /root/reference/PAPER.md (the paper's text).  What each call computes:
+ *   - governing equations, flux form: Sec. 2.1 Eq. 1-3 (L63-L67), EOS Eq. 7 (L80-L82),
+ *     perturbation pressure and buoyancy (L84), stress tensor Eq. 9 (L100-L104);
+ *   - RK3 stages Eq. 10-13 (L120-L136) with acoustic substepping (L138-L144, L170) in
+ *     the perturbation form of Appendix A (L577-L593);
+ *   - Arakawa C-grid, terrain-following height coordinate, node heights (L178-L180);
+ *   - advective fluxes and the interpolation stencils Eq. 17-21 (L196-L215);
+ *   - periodic lateral boundaries (L229), slip-wall lids (L231, Table C1).
+ * Where the paper is silent the discrete reading is "D0", listed in DESIGN.md.
+ *
+ * Conventions.
+ *   - Every function returns an int status (ERF_OK = 0, negative = error), never throws,
+ *     never prints.  erf_strerror() maps a status to a static string.
+ *   - "DEVICE" pointers are CUDA global-memory addresses valid on the current device;
+ *     "HOST" pointers are ordinary process memory.  The caller owns every pointer it
+ *     passes; the library copies what it needs during the call's enqueued work and never
+ *     retains a caller pointer after that work has run on the stream.
+ *   - Field layout at the boundary: dense, unpadded, x fastest.  rho, rhou, rhov,
+ *     rhotheta are [nz][ny][nx]; rhow is [nz+1][ny][nx].  rhou[k][j][i] sits on the low-x
+ *     face of cell i, rhov[k][j][i] on the low-y face of cell j, rhow[k][j][i] on the
+ *     low-z face of level k.  All fp64.
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *     Calls only enqueue work on that stream (erf_create and erf_destroy also
+ *     synchronise it).  Using one context from two streams concurrently is undefined.
+ *   - There is no CPU fallback: every call fails with ERF_ECUDA if no CUDA device works.
+ */
+#ifndef ERF_B200_H
+#define ERF_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ERF_OK 0
+#define ERF_EINVAL (-1)       /* null pointer, non-positive size, bad order / substep count / dt */
+#define ERF_EUNSUPPORTED (-2) /* non-periodic lateral boundary                                   */
+#define ERF_ENOMEM (-3)       /* host or device allocation failed                                */
+#define ERF_ECUDA (-4)        /* a CUDA runtime call or kernel launch failed (sticky)            */
+
+typedef struct erf_ctx erf_ctx; /* opaque; owns all internal device memory */
+
+typedef struct {
+  int nx, ny, nz;             /* cells */
+  double dx, dy;              /* m, uniform (L178) */
+  int periodic_x, periodic_y; /* must both be 1 (L229), else ERF_EUNSUPPORTED */
+} erf_grid;
+
+typedef struct {
+  const double *z_nodes;   /* DEVICE [(nz+1)][(ny+1)][(nx+1)] node heights, m: terrain lives at
+                              nodes, deformation vertical only (L178).  Column nx must repeat
+                              column 0 and row ny row 0 (periodic).  NULL => flat grid.        */
+  const double *z_levels;  /* HOST [(nz+1)] face heights of a flat (possibly stretched, L180)
+                              grid; used only when z_nodes is NULL.                             */
+  const double *rho0;      /* DEVICE base-state density (L84): [nz][ny][nx], or [nz] if base_is_1d */
+  const double *rhotheta0; /* DEVICE base-state rho0*theta0, same shape; p0 and pi0 follow from
+                              Eq. 7 (L80)                                                        */
+  int base_is_1d;
+} erf_metrics;
+
+typedef struct {
+  double Rd, cp, g, p00;        /* 287, 1004.5, 9.81, 1e5 in the paper (L82)                  */
+  int adv_order_h, adv_order_v; /* 2..6: Eq. 17-21 (L198-L215); horizontal / vertical (L215)  */
+  int diffusion;                /* 0 none, 1 constant nu (L104), 2 Smagorinsky-Lilly (L104)   */
+  double nu, alpha_theta;       /* m^2/s, kinematic; mu = rho*nu, K = rho*alpha (+ SGS part)  */
+  double Cs, Pr_t;              /* Smagorinsky constant (Table C1), turbulent Prandtl number  */
+  double beta_s;                /* off-centring of the vertically implicit solve, 0.1 (L591)  */
+  double beta_d;                /* divergence damping (L144), 0.1; 0 switches it off          */
+  int substep_mode;             /* 1 semi-implicit substepping (default);
+                                   0 none: S_stage = S^n + dt_s f(S) (L140), a test mode      */
+} erf_params;
+
+/* Build a context: copies grid/params, derives all metric terms from the node heights
+ * (S0), the base-state p0 and pi0 from Eq. 7, allocates every work array.
+ * The metrics pointers are read during the call only.  Synchronises cuda_stream. */
+int erf_create(const erf_grid *grid, const erf_metrics *metrics, const erf_params *params,
+               void *cuda_stream, erf_ctx **out);
+
+/* Copy a state S^n = (rho, rho*u, rho*v, rho*w, rho*theta) from DEVICE arrays into the
+ * context and impose the kinematic lid values of rho*w (Omega = 0 at k = 0 and k = nz). */
+int erf_set_state(erf_ctx *ctx, const double *rho, const double *rhou, const double *rhov,
+                  const double *rhow, const double *rhotheta, void *cuda_stream);
+
+/* Advance the state by one RK3 step of size dt (Eq. 11-13).  n_acoustic = number
+ * of acoustic substeps per dt: even and >= 2 (L170); RK stage 1 takes one substep of dt/3,
+ * stage 2 n_acoustic/2 and stage 3 n_acoustic substeps of dt/n_acoustic.  Enqueue only. */
+int erf_rk3_step(erf_ctx *ctx, double dt, int n_acoustic, void *cuda_stream);
+
+/* Copy the current state into DEVICE arrays (any of them may be NULL = skip). */
+int erf_get_state(erf_ctx *ctx, double *rho, double *rhou, double *rhov, double *rhow,
+                  double *rhotheta, void *cuda_stream);
+
+/* Free everything; erf_destroy(NULL) is a no-op. */
+void erf_destroy(erf_ctx *ctx);
+
+const char *erf_strerror(int code);
+
+/* ---- per-operator entry points (used by the parity tests and the profiler) ---- */
+
+/* The slow right-hand side f(S) of Eq. 1-3 for the CURRENT state: advection (L196-L215),
+ * diffusion (Eq. 9), pressure gradient and buoyancy (L84).  DEVICE outputs, dense;
+ * R_W is [nz+1][ny][nx] with zero lids.  Any output may be NULL. */
+int erf_slow_rhs(erf_ctx *ctx, double *R_rho, double *R_U, double *R_V, double *R_W,
+                 double *R_Theta, void *cuda_stream);
+
+/* Appendix A: n substeps of size dtau about the CURRENT state as stage state S^t, given the
+ * slow tendencies R and the perturbation S'' (DEVICE, dense, in/out; W'' is [nz+1]). */
+int erf_acoustic(erf_ctx *ctx, double dtau, int n, const double *R_rho, const double *R_U,
+                 const double *R_V, const double *R_W, const double *R_Theta, double *rho_pp,
+                 double *U_pp, double *V_pp, double *W_pp, double *Theta_pp, void *cuda_stream);
+
+/* Select the kernel path: ERF_PATH_AUTO picks the fused kernels where they apply;
+ * ERF_PATH_GENERAL forces the unfused, terrain-general kernels (one kernel per operator,
+ * every intermediate field in HBM), kept as an on-device cross-check of the fused ones. */
+#define ERF_PATH_AUTO 0
+#define ERF_PATH_GENERAL 1
+int erf_set_path(erf_ctx *ctx, int path);
+
+/* Number of kernels launched by this context so far (for bench.py's gpu_launches). */
+long long erf_launch_count(const erf_ctx *ctx);
+
+/* Device bytes owned by the context. */
+long long erf_device_bytes(const erf_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

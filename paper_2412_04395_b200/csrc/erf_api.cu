@@ -1,0 +1,279 @@
+// erf_api.cu -- the C-ABI of liberf_b200.so (include/erf_b200.h): context, state copies,
+// the RK3 driver (Eq. 11-13; substep schedule L170).
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "erf_ctx.cuh"
+#include "fused.cuh"
+
+using namespace erfb;
+
+double *erf_ctx::alloc(size_t n) {
+  void *p = nullptr;
+  if (cudaMalloc(&p, n * sizeof(double)) != cudaSuccess) {
+    cudaGetLastError();
+    status = ERF_ENOMEM;
+    return nullptr;
+  }
+  if (cudaMemset(p, 0, n * sizeof(double)) != cudaSuccess) {
+    status = ERF_ECUDA;
+    cudaFree(p);
+    return nullptr;
+  }
+  allocs.push_back(p);
+  bytes += (long long)(n * sizeof(double));
+  return (double *)p;
+}
+
+static int check(erf_ctx *c) {
+  if (c->status != ERF_OK) return c->status;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) c->status = ERF_ECUDA;
+  return c->status;
+}
+
+extern "C" const char *erf_strerror(int code) {
+  switch (code) {
+    case ERF_OK: return "ok";
+    case ERF_EINVAL: return "invalid argument";
+    case ERF_EUNSUPPORTED: return "unsupported configuration (lateral boundaries must be periodic)";
+    case ERF_ENOMEM: return "out of memory";
+    case ERF_ECUDA: return "CUDA error";
+    default: return "unknown error";
+  }
+}
+
+extern "C" void erf_destroy(erf_ctx *c) {
+  if (!c) return;
+  cudaDeviceSynchronize();
+  fused_release(c);
+  for (void *p : c->allocs) cudaFree(p);
+  delete c;
+}
+
+extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_params *p, void *stream,
+                          erf_ctx **out) {
+  if (!g || !m || !p || !out) return ERF_EINVAL;
+  *out = nullptr;
+  if (g->nx < 1 || g->ny < 1 || g->nz < 1 || !(g->dx > 0) || !(g->dy > 0)) return ERF_EINVAL;
+  if (!g->periodic_x || !g->periodic_y) return ERF_EUNSUPPORTED;
+  if (!m->rho0 || !m->rhotheta0 || (!m->z_nodes && !m->z_levels)) return ERF_EINVAL;
+  if (p->adv_order_h < 2 || p->adv_order_h > 6 || p->adv_order_v < 2 || p->adv_order_v > 6) return ERF_EINVAL;
+  if (p->diffusion < 0 || p->diffusion > 2 || (p->substep_mode != 0 && p->substep_mode != 1)) return ERF_EINVAL;
+  if (!(p->cp > p->Rd) || !(p->Rd > 0) || !(p->p00 > 0)) return ERF_EINVAL;
+  if (p->diffusion == 2 && !(p->Pr_t > 0)) return ERF_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return ERF_ECUDA;
+  }
+  cudaStream_t st = (cudaStream_t)stream;
+  erf_ctx *c = new (std::nothrow) erf_ctx();
+  if (!c) return ERF_ENOMEM;
+  c->nx = g->nx; c->ny = g->ny; c->nz = g->nz;
+  c->NW = (size_t)g->nx * g->ny * (g->nz + 1);
+  c->p = *p;
+  c->path = ERF_PATH_AUTO;
+  c->status = ERF_OK;
+  c->launches = 0;
+  c->bytes = 0;
+  c->diff_alloc = false;
+  c->zl_dev = nullptr;
+  memset(&c->diff, 0, sizeof(c->diff));
+  memset(&c->ac, 0, sizeof(c->ac));
+
+  View &v = c->v;
+  memset(&v, 0, sizeof(v));
+  v.nx = g->nx; v.ny = g->ny; v.nz = g->nz;
+  v.oh = p->adv_order_h; v.ov = p->adv_order_v; v.diffusion = p->diffusion;
+  v.flat = m->z_nodes ? 0 : 1;
+  v.dx = g->dx; v.dy = g->dy;
+  v.Rd = p->Rd; v.cp = p->cp; v.g = p->g; v.p00 = p->p00;
+  v.gam = p->cp / (p->cp - p->Rd);    // L82
+  v.rdocv = p->Rd / (p->cp - p->Rd);  // Rd/cv
+  v.nu = p->diffusion >= 1 ? p->nu : 0.0;
+  v.alpha = p->diffusion >= 1 ? p->alpha_theta : 0.0;
+  v.Cs = p->Cs; v.Prt = p->Pr_t; v.beta_s = p->beta_s; v.beta_d = p->beta_d;
+
+  double **geo[] = {&c->zxf, &c->zyf, &c->zw, &c->hx, &c->hy, &c->hc, &c->zc, &c->hw, &c->hu, &c->hv,
+                    &c->sxw, &c->syw, &c->sxu, &c->syv, &c->rho0, &c->Th0, &c->p0, &c->pi0,
+                    &c->theta_t, &c->pi_t, &c->prim.theta, &c->prim.pp, &c->prim.pi, &c->prim.u,
+                    &c->prim.v, &c->prim.w, &c->Om_slow, &c->ac.Om, &c->ac.Th_prev, &c->ac.Thd,
+                    &c->ac.om, &c->ac.Ttil, &c->ac.rtil, &c->ac.cpr, &c->ac.dpr};
+  for (auto pp : geo) *pp = c->alloc(c->NW);
+  for (int f = 0; f < 5; f++) {
+    c->S.f[f] = c->alloc(c->NW);
+    c->St.f[f] = c->alloc(c->NW);
+    c->R.f[f] = c->alloc(c->NW);
+    c->P.f[f] = c->alloc(c->NW);
+  }
+  if (c->status != ERF_OK) {
+    int rc = c->status;
+    erf_destroy(c);
+    return rc;
+  }
+  v.zw = c->zw; v.hx = c->hx; v.hy = c->hy; v.hc = c->hc; v.zc = c->zc; v.hw = c->hw;
+  v.hu = c->hu; v.hv = c->hv; v.sxw = c->sxw; v.syw = c->syw; v.sxu = c->sxu; v.syv = c->syv;
+  v.rho0 = c->rho0; v.Th0 = c->Th0; v.p0 = c->p0; v.pi0 = c->pi0;
+
+  // geometry from node heights (S0)
+  gen::NodeH Z;
+  Z.zn = m->z_nodes; Z.zl = nullptr; Z.nx = g->nx; Z.ny = g->ny;
+  if (!m->z_nodes) {
+    c->zl_dev = c->alloc(g->nz + 1);
+    if (!c->zl_dev) { int rc = c->status; erf_destroy(c); return rc; }
+    cudaMemcpyAsync(c->zl_dev, m->z_levels, (g->nz + 1) * sizeof(double), cudaMemcpyHostToDevice, st);
+    Z.zl = c->zl_dev;
+  }
+  {
+    View vv = v;
+    double *zxf = c->zxf, *zyf = c->zyf, *zw = c->zw, *hx = c->hx, *hy = c->hy, *hc = c->hc, *zc = c->zc;
+    double *hw = c->hw, *hu = c->hu, *hv = c->hv, *sxu = c->sxu, *syv = c->syv, *sxw = c->sxw, *syw = c->syw;
+    double *rho0 = c->rho0, *Th0 = c->Th0, *p0 = c->p0, *pi0 = c->pi0;
+    const double *r0in = m->rho0, *t0in = m->rhotheta0;
+    int b1d = m->base_is_1d;
+    launch_cells(c, st, g->nz + 1, [=] __device__(int i, int j, int k) { gen::geo_faces(vv, Z, zxf, zyf, zw, i, j, k); });
+    launch_cells(c, st, g->nz, [=] __device__(int i, int j, int k) { gen::geo_cells(vv, zxf, zyf, zw, hx, hy, hc, zc, i, j, k); });
+    launch_cells(c, st, g->nz + 1, [=] __device__(int i, int j, int k) {
+      gen::geo_derived(vv, zxf, zyf, hc, zc, hw, hu, hv, sxu, syv, sxw, syw, i, j, k);
+    });
+    launch_cells(c, st, g->nz, [=] __device__(int i, int j, int k) {
+      gen::base_state(vv, r0in, t0in, b1d, rho0, Th0, p0, pi0, i, j, k);
+    });
+  }
+  int rc = fused_setup(c, m, st);
+  if (rc == ERF_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = ERF_ECUDA;
+  if (rc == ERF_OK) rc = check(c);
+  if (rc != ERF_OK) {
+    erf_destroy(c);
+    return rc;
+  }
+  *out = c;
+  return ERF_OK;
+}
+
+extern "C" int erf_set_state(erf_ctx *c, const double *rho, const double *rhou, const double *rhov,
+                             const double *rhow, const double *rhotheta, void *stream) {
+  if (!c || !rho || !rhou || !rhov || !rhow || !rhotheta) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  cudaStream_t st = (cudaStream_t)stream;
+  size_t nc = (size_t)c->nx * c->ny * c->nz * sizeof(double);
+  cudaMemcpyAsync(c->S.f[RHO], rho, nc, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(c->S.f[UU], rhou, nc, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(c->S.f[VV], rhov, nc, cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(c->S.f[WW], rhow, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(c->S.f[TH], rhotheta, nc, cudaMemcpyDeviceToDevice, st);
+  general_lids(c, c->S, st);
+  return check(c);
+}
+
+extern "C" int erf_get_state(erf_ctx *c, double *rho, double *rhou, double *rhov, double *rhow,
+                             double *rhotheta, void *stream) {
+  if (!c) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  cudaStream_t st = (cudaStream_t)stream;
+  size_t nc = (size_t)c->nx * c->ny * c->nz * sizeof(double);
+  if (rho) cudaMemcpyAsync(rho, c->S.f[RHO], nc, cudaMemcpyDeviceToDevice, st);
+  if (rhou) cudaMemcpyAsync(rhou, c->S.f[UU], nc, cudaMemcpyDeviceToDevice, st);
+  if (rhov) cudaMemcpyAsync(rhov, c->S.f[VV], nc, cudaMemcpyDeviceToDevice, st);
+  if (rhow) cudaMemcpyAsync(rhow, c->S.f[WW], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  if (rhotheta) cudaMemcpyAsync(rhotheta, c->S.f[TH], nc, cudaMemcpyDeviceToDevice, st);
+  return check(c);
+}
+
+extern "C" int erf_set_path(erf_ctx *c, int path) {
+  if (!c || (path != ERF_PATH_AUTO && path != ERF_PATH_GENERAL)) return ERF_EINVAL;
+  c->path = path;
+  return ERF_OK;
+}
+
+extern "C" long long erf_launch_count(const erf_ctx *c) { return c ? c->launches : 0; }
+extern "C" long long erf_device_bytes(const erf_ctx *c) { return c ? c->bytes : 0; }
+
+static bool use_fused(const erf_ctx *c) { return c->path == ERF_PATH_AUTO && fused_available(c); }
+
+// substep schedule of RK stage s (L170): one substep of dt/3 in stage 1, then ns/2 and ns of dt/ns
+static void schedule(int stage, double dt, int ns, int *nsub, double *dtau, double *dts) {
+  if (stage == 1) { *nsub = 1; *dtau = dt / 3.0; *dts = dt / 3.0; }
+  else if (stage == 2) { *nsub = ns / 2; *dtau = dt / ns; *dts = dt / 2.0; }
+  else { *nsub = ns; *dtau = dt / ns; *dts = dt; }
+}
+
+extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream) {
+  if (!c || !(dt > 0.0)) return ERF_EINVAL;
+  if (c->p.substep_mode == 1 && (n_acoustic < 2 || (n_acoustic & 1))) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (use_fused(c)) {
+    fused_rk3_step(c, dt, n_acoustic, st);
+    return check(c);
+  }
+  for (int f = 0; f < 5; f++)  // S^t = S^n
+    cudaMemcpyAsync(c->St.f[f], c->S.f[f], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  for (int stage = 1; stage <= 3; stage++) {
+    int nsub; double dtau, dts;
+    schedule(stage, dt, n_acoustic, &nsub, &dtau, &dts);
+    general_slow_rhs(c, c->St, st);  // f(S^t), every stage (L140)
+    if (c->p.substep_mode == 0) {
+      F5 S = c->S, St = c->St, R = c->R;
+      View v = c->v;
+      launch_cells(c, st, c->nz + 1, [=] __device__(int i, int j, int k) {
+        size_t a = IX(v, i, j, k);
+        for (int f = 0; f < 5; f++)
+          if (f == WW || k < v.nz) St.f[f][a] = S.f[f][a] + dts * R.f[f][a];
+      });
+      general_lids(c, c->St, st);
+    } else {
+      general_stage_init(c, st);  // S'' = S^n - S^t (L581) [R:G7]
+      general_acoustic(c, c->St, dtau, nsub, st);
+      general_stage_finish(c, st);  // S = S^t + S'' (L593), lids
+    }
+  }
+  for (int f = 0; f < 5; f++) {
+    double *t = c->S.f[f];
+    c->S.f[f] = c->St.f[f];
+    c->St.f[f] = t;
+  }
+  return check(c);
+}
+
+extern "C" int erf_slow_rhs(erf_ctx *c, double *R_rho, double *R_U, double *R_V, double *R_W, double *R_Theta,
+                            void *stream) {
+  if (!c) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (use_fused(c)) fused_slow_rhs(c, c->S, st);
+  else general_slow_rhs(c, c->S, st);
+  size_t nc = (size_t)c->nx * c->ny * c->nz * sizeof(double);
+  double *out[5] = {R_rho, R_U, R_V, R_W, R_Theta};
+  for (int f = 0; f < 5; f++)
+    if (out[f])
+      cudaMemcpyAsync(out[f], c->R.f[f], f == WW ? c->NW * sizeof(double) : nc, cudaMemcpyDeviceToDevice, st);
+  return check(c);
+}
+
+extern "C" int erf_acoustic(erf_ctx *c, double dtau, int n, const double *R_rho, const double *R_U,
+                            const double *R_V, const double *R_W, const double *R_Theta, double *rho_pp,
+                            double *U_pp, double *V_pp, double *W_pp, double *Theta_pp, void *stream) {
+  if (!c || !R_rho || !R_U || !R_V || !R_W || !R_Theta || !rho_pp || !U_pp || !V_pp || !W_pp || !Theta_pp)
+    return ERF_EINVAL;
+  if (!(dtau > 0.0) || n < 0) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  cudaStream_t st = (cudaStream_t)stream;
+  size_t nc = (size_t)c->nx * c->ny * c->nz * sizeof(double), nw = c->NW * sizeof(double);
+  // stage constants theta^t, pi^t from the current state (the slow-RHS kernels produce them)
+  if (use_fused(c)) fused_slow_rhs(c, c->S, st);
+  else general_slow_rhs(c, c->S, st);
+  const double *Rin[5] = {R_rho, R_U, R_V, R_W, R_Theta};
+  double *Pio[5] = {rho_pp, U_pp, V_pp, W_pp, Theta_pp};
+  for (int f = 0; f < 5; f++) {
+    cudaMemcpyAsync(c->R.f[f], Rin[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(c->P.f[f], Pio[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
+  }
+  if (use_fused(c)) fused_acoustic(c, c->S, dtau, n, st);
+  else general_acoustic(c, c->S, dtau, n, st);
+  for (int f = 0; f < 5; f++)
+    cudaMemcpyAsync(Pio[f], c->P.f[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
+  return check(c);
+}

@@ -1,0 +1,99 @@
+// erf_ctx.cuh -- the context behind the opaque erf_ctx handle, and launch helpers.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <vector>
+
+#include "../../include/erf_b200.h"
+#include "erf_view.cuh"
+#include "general_cells.cuh"
+
+namespace erfb {
+
+struct F5 {
+  double *f[5];
+};
+
+}  // namespace erfb
+
+struct erf_ctx {
+  int nx, ny, nz;
+  size_t NW;  // elements of one 3-D array: nx*ny*(nz+1)
+  erf_params p;
+  erfb::View v;
+  int path;
+  int status;  // sticky error
+  long long launches;
+  long long bytes;
+  std::vector<void *> allocs;
+
+  // geometry (owned; v holds const aliases)
+  double *zxf, *zyf, *zw, *hx, *hy, *hc, *zc, *hw, *hu, *hv, *sxw, *syw, *sxu, *syv;
+  double *rho0, *Th0, *p0, *pi0;
+  double *zl_dev;  // [(nz+1)] flat level heights (device) or null
+
+  erfb::F5 S, St, R, P;  // S^n, stage state S^t, slow tendencies, perturbation S''
+  double *theta_t, *pi_t;
+  erfb::gen::Prim prim;  // general path intermediates
+  double *Om_slow;      // contravariant flux of the stage state (general path)
+  erfb::gen::Diff diff;
+  bool diff_alloc;
+  erfb::gen::Acou ac;
+
+  double *alloc(size_t n);  // zero-initialised device doubles; null on failure (sets status)
+};
+
+#ifdef ERF_HOSTCHECK  // developer-only host emulation of the launches (never built into the library)
+#include "host_launch.h"
+#else
+namespace erfb {
+
+template <class F>
+__global__ void k_cells(int nx, int ny, int nlev, F f) {
+  size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  size_t n = (size_t)nx * ny * nlev;
+  if (idx >= n) return;
+  int i = (int)(idx % nx);
+  size_t r = idx / nx;
+  int j = (int)(r % ny);
+  int k = (int)(r / ny);
+  f(i, j, k);
+}
+
+template <class F>
+__global__ void k_columns(int nx, int ny, F f) {
+  size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= (size_t)nx * ny) return;
+  f((int)(idx % nx), (int)(idx / nx));
+}
+
+template <class F>
+inline void launch_cells(erf_ctx *c, cudaStream_t st, int nlev, F f) {
+  size_t n = (size_t)c->nx * c->ny * nlev;
+  if (n == 0) return;
+  unsigned blocks = (unsigned)((n + 255) / 256);
+  k_cells<<<blocks, 256, 0, st>>>(c->nx, c->ny, nlev, f);
+  c->launches++;
+}
+
+template <class F>
+inline void launch_columns(erf_ctx *c, cudaStream_t st, F f) {
+  size_t n = (size_t)c->nx * c->ny;
+  unsigned blocks = (unsigned)((n + 127) / 128);
+  k_columns<<<blocks, 128, 0, st>>>(c->nx, c->ny, f);
+  c->launches++;
+}
+
+}  // namespace erfb
+#endif
+
+namespace erfb {
+
+// general path (k_general.cu)
+void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st);  // fills c->R, theta_t, pi_t
+void general_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st);  // c->P in/out
+void general_stage_init(erf_ctx *c, cudaStream_t st);    // P = S - St
+void general_stage_finish(erf_ctx *c, cudaStream_t st);  // St += P, lids
+void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st);
+
+}  // namespace erfb

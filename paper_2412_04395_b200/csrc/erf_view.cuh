@@ -1,0 +1,51 @@
+// erf_view.cuh -- plain-data view of a context that kernels take by value, and the
+// index helpers every kernel uses.  Internal to liberf_b200.so.
+//
+// HBM layout: every 3-D field is dense, x fastest, [nlev][ny][nx] with nlev = nz (cell
+// and horizontal-face fields) or nz+1 (w-face fields); all are allocated with nz+1
+// levels.  There are no ghost cells: the periodic lateral boundary is
+// an index wrap at load time, so no halo-fill pass ever touches HBM.
+#pragma once
+#include <cstddef>
+
+#ifdef __CUDACC__
+#define ERF_HD __host__ __device__ __forceinline__
+#else
+#define ERF_HD inline
+#endif
+
+namespace erfb {
+
+enum { RHO = 0, UU = 1, VV = 2, WW = 3, TH = 4 };
+
+struct View {
+  int nx, ny, nz;
+  int oh, ov, diffusion;
+  int flat, pad_;
+  double dx, dy;
+  double Rd, cp, g, p00, gam, rdocv;
+  double nu, alpha, Cs, Prt, beta_s, beta_d;
+  // geometry (S0), 3-D, levels as noted
+  const double *zw;        // 0..nz   w-face centre height
+  const double *hx, *hy;   // 0..nz-1 x-/y-face heights
+  const double *hc, *zc;   // 0..nz-1 cell thickness, centre height
+  const double *hw;        // 1..nz-1 centre-to-centre spacing
+  const double *hu, *hv;   // 0..nz-1 U/V control-volume thickness
+  const double *sxw, *syw; // 0..nz   slopes of the w-faces
+  const double *sxu, *syv; // 0..nz-1 slopes of the centre surface at u-/v-points
+  // base state, 3-D
+  const double *rho0, *Th0, *p0, *pi0;
+};
+
+ERF_HD int wrapi(int a, int n) {
+  while (a < 0) a += n;
+  while (a >= n) a -= n;
+  return a;
+}
+
+// periodic index into a dense [.][ny][nx] field
+ERF_HD size_t IX(const View &c, int i, int j, int k) {
+  return ((size_t)k * c.ny + wrapi(j, c.ny)) * c.nx + wrapi(i, c.nx);
+}
+
+}  // namespace erfb

@@ -1,0 +1,116 @@
+// k_general.cu -- the GENERAL path: one kernel per operator pass, all intermediates in HBM.
+// Serves terrain-following grids and cross-checks the fused kernels on the device.
+#include "erf_ctx.cuh"
+
+namespace erfb {
+
+static bool ensure_diff(erf_ctx *c) {
+  if (c->diff_alloc) return true;
+  gen::Diff &d = c->diff;
+  double **all[] = {&d.mu, &d.K, &d.S11, &d.S22, &d.S33, &d.S12, &d.S13, &d.S23, &d.qu, &d.qv,
+                    &d.t11, &d.t22, &d.t33, &d.t12, &d.t13, &d.t23, &d.q11, &d.q22, &d.q12,
+                    &d.q13, &d.q23, &d.qth, &d.ze12, &d.Fx, &d.Fy, &d.Fz};
+  for (auto p : all) {
+    *p = c->alloc(c->NW);
+    if (!*p) return false;
+  }
+  c->diff_alloc = true;
+  return true;
+}
+
+void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st) {
+  View v = c->v;
+  const double *U = S.f[UU], *V = S.f[VV];
+  double *W = S.f[WW];
+  launch_columns(c, st, [=] __device__(int i, int j) { gen::lids(v, U, V, W, i, j); });
+}
+
+void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st) {
+  View v = c->v;
+  const int nz = c->nz;
+  gen::Prim q = c->prim;
+  F5 Sv = S, R = c->R;
+  double *Om = c->Om_slow;
+  launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::primitives(v, Sv.f, q, i, j, k); });
+  launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) {
+    Om[IX(v, i, j, k)] = gen::omega_at(v, Sv.f[UU], Sv.f[VV], Sv.f[WW], i, j, k);
+  });
+  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::advect_cell(v, Sv.f, Om, q, R.f, i, j, k); });
+  launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::advect_wface(v, Sv.f, Om, q, R.f, i, j, k); });
+  if (c->p.diffusion != 0) {
+    if (!ensure_diff(c)) return;
+    gen::Diff d = c->diff;
+    const double *rho = S.f[RHO];
+    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::diff_pass1(v, q, d, i, j, k); });
+    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::diff_pass2(v, q, d, i, j, k); });
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass3(v, rho, d, i, j, k); });
+    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::diff_pass4(v, d, i, j, k); });
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass5(v, q, d, i, j, k); });
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass6(v, q, d, R.f, i, j, k); });
+    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::diff_pass7(v, d, i, j, k); });
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass8(v, d, R.f, i, j, k); });
+  }
+  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::pgbuoy_cell(v, Sv.f, q, R.f, i, j, k); });
+  // stage constants for the substeps: theta^t, pi^t
+  cudaMemcpyAsync(c->theta_t, q.theta, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  cudaMemcpyAsync(c->pi_t, q.pi, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+}
+
+void general_stage_init(erf_ctx *c, cudaStream_t st) {
+  F5 S = c->S, St = c->St, P = c->P;
+  View v = c->v;
+  launch_cells(c, st, c->nz + 1, [=] __device__(int i, int j, int k) {
+    size_t a = IX(v, i, j, k);
+    if (k < v.nz) {
+      P.f[RHO][a] = S.f[RHO][a] - St.f[RHO][a];
+      P.f[UU][a] = S.f[UU][a] - St.f[UU][a];
+      P.f[VV][a] = S.f[VV][a] - St.f[VV][a];
+      P.f[TH][a] = S.f[TH][a] - St.f[TH][a];
+    }
+    P.f[WW][a] = S.f[WW][a] - St.f[WW][a];
+  });
+}
+
+void general_stage_finish(erf_ctx *c, cudaStream_t st) {
+  F5 St = c->St, P = c->P;
+  View v = c->v;
+  launch_cells(c, st, c->nz + 1, [=] __device__(int i, int j, int k) {
+    size_t a = IX(v, i, j, k);
+    if (k < v.nz) {
+      St.f[RHO][a] += P.f[RHO][a];
+      St.f[UU][a] += P.f[UU][a];
+      St.f[VV][a] += P.f[VV][a];
+      St.f[TH][a] += P.f[TH][a];
+    }
+    St.f[WW][a] += P.f[WW][a];
+  });
+  general_lids(c, c->St, st);
+}
+
+// n substeps of size dtau about the stage state St (theta_t, pi_t, R, P set by the caller)
+void general_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st) {
+  View v = c->v;
+  const int nz = c->nz;
+  gen::Acou A = c->ac;
+  A.theta_t = c->theta_t;
+  A.pi_t = c->pi_t;
+  A.Th_t = St.f[TH];
+  for (int m = 0; m < 5; m++) {
+    A.R[m] = c->R.f[m];
+    A.P[m] = c->P.f[m];
+  }
+  // Omega'' of the initial S''; Theta''_prev = Theta''
+  launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) {
+    size_t a = IX(v, i, j, k);
+    A.Om[a] = gen::omega_at(v, A.P[UU], A.P[VV], A.P[WW], i, j, k);
+    if (k < v.nz) A.Th_prev[a] = A.P[TH][a];
+  });
+  for (int s = 0; s < n; s++) {
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::ac_damp(v, A, i, j, k); });
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::ac_horiz(v, A, dtau, i, j, k); });
+    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::ac_slope(v, A, i, j, k); });
+    launch_columns(c, st, [=] __device__(int i, int j) { gen::ac_column(v, A, dtau, i, j); });
+  }
+}
+
+}  // namespace erfb
