@@ -122,6 +122,17 @@ int erf_set_path(erf_ctx *ctx, int path);
 /* Number of kernels launched by this context so far (for bench.py's gpu_launches). */
 long long erf_launch_count(const erf_ctx *ctx);
 
+/* Per-kernel device timing.  erf_set_timing(ctx, 1) makes every subsequent call bracket each
+ * kernel (or group of small kernels) with CUDA events on the call's stream; erf_get_timing
+ * synchronises, and returns for class id (0 <= id < ERF_TIMING_CLASSES) the number of bracketed
+ * launches and their total device time in milliseconds since the last erf_reset_timing.
+ * erf_timing_name(id) is a static string.  Off by default (no events are recorded). */
+#define ERF_TIMING_CLASSES 8
+int erf_set_timing(erf_ctx *ctx, int on);
+int erf_get_timing(erf_ctx *ctx, int id, long long *launches, double *total_ms);
+int erf_reset_timing(erf_ctx *ctx);
+const char *erf_timing_name(int id);
+
 /* Device bytes owned by the context. */
 long long erf_device_bytes(const erf_ctx *ctx);
 

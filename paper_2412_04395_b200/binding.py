@@ -22,7 +22,8 @@ ERF_PATH_AUTO, ERF_PATH_GENERAL = 0, 1
 
 EXPORTS = ["erf_create", "erf_set_state", "erf_rk3_step", "erf_get_state", "erf_destroy",
            "erf_strerror", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_launch_count",
-           "erf_device_bytes"]
+           "erf_device_bytes", "erf_set_timing", "erf_get_timing", "erf_reset_timing", "erf_timing_name"]
+ERF_TIMING_CLASSES = 8
 
 _dp = C.c_void_p
 
@@ -82,6 +83,11 @@ def load(path: str | None = None):
     L.erf_launch_count.restype = C.c_longlong
     L.erf_device_bytes.argtypes = [C.c_void_p]
     L.erf_device_bytes.restype = C.c_longlong
+    L.erf_set_timing.argtypes = [C.c_void_p, C.c_int]
+    L.erf_reset_timing.argtypes = [C.c_void_p]
+    L.erf_get_timing.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
+    L.erf_timing_name.argtypes = [C.c_int]
+    L.erf_timing_name.restype = C.c_char_p
     _lib = L
     return L
 
@@ -156,6 +162,24 @@ def erf_launch_count(h):
 
 def erf_device_bytes(h):
     return int(load().erf_device_bytes(h))
+
+
+def erf_set_timing(h, on):
+    _ck(load().erf_set_timing(h, int(bool(on))), "erf_set_timing")
+
+
+def erf_reset_timing(h):
+    _ck(load().erf_reset_timing(h), "erf_reset_timing")
+
+
+def erf_get_timing(h, idx):
+    n, ms = C.c_longlong(), C.c_double()
+    _ck(load().erf_get_timing(h, int(idx), C.byref(n), C.byref(ms)), "erf_get_timing")
+    return n.value, ms.value
+
+
+def erf_timing_name(idx):
+    return load().erf_timing_name(int(idx)).decode()
 
 
 def make_params(par: dict) -> erf_params:
@@ -251,6 +275,21 @@ class Dycore:
 
     def set_path(self, path):
         erf_set_path(self._h, path)
+
+    def set_timing(self, on):
+        erf_set_timing(self._h, on)
+
+    def reset_timing(self):
+        erf_reset_timing(self._h)
+
+    def timing(self):
+        """{class name: (launch groups, total device ms)} since the last reset."""
+        out = {}
+        for i in range(ERF_TIMING_CLASSES):
+            n, ms = erf_get_timing(self._h, i)
+            if n:
+                out[erf_timing_name(i)] = (n, ms)
+        return out
 
     @property
     def launch_count(self):

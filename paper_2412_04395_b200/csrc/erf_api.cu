@@ -48,6 +48,10 @@ extern "C" void erf_destroy(erf_ctx *c) {
   if (!c) return;
   cudaDeviceSynchronize();
   fused_release(c);
+#ifndef ERF_HOSTCHECK
+  for (auto &s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+  for (auto e : c->event_pool) cudaEventDestroy(e);
+#endif
   for (void *p : c->allocs) cudaFree(p);
   delete c;
 }
@@ -80,6 +84,8 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   c->bytes = 0;
   c->diff_alloc = false;
   c->zl_dev = nullptr;
+  c->timing = false;
+  for (int i = 0; i < ERF_TIMING_CLASSES; i++) { c->t_calls[i] = 0; c->t_ms[i] = 0.0; }
   memset(&c->diff, 0, sizeof(c->diff));
   memset(&c->ac, 0, sizeof(c->ac));
 
@@ -188,6 +194,50 @@ extern "C" int erf_set_path(erf_ctx *c, int path) {
   return ERF_OK;
 }
 
+static void drain_timing(erf_ctx *c) {
+#ifndef ERF_HOSTCHECK
+  for (auto &s : c->spans) {
+    cudaEventSynchronize(s.b);
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, s.a, s.b) == cudaSuccess) {
+      c->t_ms[s.id] += ms;
+      c->t_calls[s.id]++;
+    }
+    c->event_pool.push_back(s.a);
+    c->event_pool.push_back(s.b);
+  }
+  c->spans.clear();
+#endif
+}
+
+extern "C" int erf_set_timing(erf_ctx *c, int on) {
+  if (!c) return ERF_EINVAL;
+  c->timing = on != 0;
+  return ERF_OK;
+}
+
+extern "C" int erf_reset_timing(erf_ctx *c) {
+  if (!c) return ERF_EINVAL;
+  drain_timing(c);
+  for (int i = 0; i < ERF_TIMING_CLASSES; i++) { c->t_calls[i] = 0; c->t_ms[i] = 0.0; }
+  return ERF_OK;
+}
+
+extern "C" int erf_get_timing(erf_ctx *c, int id, long long *launches, double *total_ms) {
+  if (!c || id < 0 || id >= ERF_TIMING_CLASSES) return ERF_EINVAL;
+  drain_timing(c);
+  if (launches) *launches = c->t_calls[id];
+  if (total_ms) *total_ms = c->t_ms[id];
+  return check(c);
+}
+
+extern "C" const char *erf_timing_name(int id) {
+  static const char *names[ERF_TIMING_CLASSES] = {"slow_rhs_general", "acoustic_general", "stage_general",
+                                                  "slow_rhs_fused", "viscosity_fused", "acoustic_fused",
+                                                  "other", "unused"};
+  return (id >= 0 && id < ERF_TIMING_CLASSES) ? names[id] : "?";
+}
+
 extern "C" long long erf_launch_count(const erf_ctx *c) { return c ? c->launches : 0; }
 extern "C" long long erf_device_bytes(const erf_ctx *c) { return c ? c->bytes : 0; }
 
@@ -214,7 +264,10 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
   for (int stage = 1; stage <= 3; stage++) {
     int nsub; double dtau, dts;
     schedule(stage, dt, n_acoustic, &nsub, &dtau, &dts);
-    general_slow_rhs(c, c->St, st);  // f(S^t), every stage (L140)
+    {
+      Timed t(c, T_SLOW_GENERAL, st);
+      general_slow_rhs(c, c->St, st);  // f(S^t), every stage (L140)
+    }
     if (c->p.substep_mode == 0) {
       F5 S = c->S, St = c->St, R = c->R;
       View v = c->v;
@@ -225,9 +278,18 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
       });
       general_lids(c, c->St, st);
     } else {
-      general_stage_init(c, st);  // S'' = S^n - S^t (L581) [R:G7]
-      general_acoustic(c, c->St, dtau, nsub, st);
-      general_stage_finish(c, st);  // S = S^t + S'' (L593), lids
+      {
+        Timed t(c, T_STAGE_GENERAL, st);
+        general_stage_init(c, st);  // S'' = S^n - S^t (L581) [R:G7]
+      }
+      {
+        Timed t(c, T_ACOUSTIC_GENERAL, st);
+        general_acoustic(c, c->St, dtau, nsub, st);
+      }
+      {
+        Timed t(c, T_STAGE_GENERAL, st);
+        general_stage_finish(c, st);  // S = S^t + S'' (L593), lids
+      }
     }
   }
   for (int f = 0; f < 5; f++) {

@@ -40,6 +40,14 @@ struct erf_ctx {
   bool diff_alloc;
   erfb::gen::Acou ac;
 
+  // per-kernel timing (erf_set_timing)
+  bool timing;
+  struct TimedSpan { int id; cudaEvent_t a, b; };
+  std::vector<TimedSpan> spans;
+  std::vector<cudaEvent_t> event_pool;
+  long long t_calls[ERF_TIMING_CLASSES];
+  double t_ms[ERF_TIMING_CLASSES];
+
   double *alloc(size_t n);  // zero-initialised device doubles; null on failure (sets status)
 };
 
@@ -88,6 +96,37 @@ inline void launch_columns(erf_ctx *c, cudaStream_t st, F f) {
 #endif
 
 namespace erfb {
+
+// timing classes
+enum { T_SLOW_GENERAL = 0, T_ACOUSTIC_GENERAL = 1, T_STAGE_GENERAL = 2, T_SLOW_FUSED = 3, T_VISC_FUSED = 4,
+       T_ACOUSTIC_FUSED = 5, T_OTHER = 6 };
+
+// brackets a region of launches on a stream with two events when timing is on
+struct Timed {
+  erf_ctx *c;
+  cudaStream_t st;
+  int idx;
+  Timed(erf_ctx *c_, int id, cudaStream_t st_) : c(c_), st(st_), idx(-1) {
+#ifndef ERF_HOSTCHECK
+    if (!c->timing) return;
+    erf_ctx::TimedSpan s;
+    s.id = id;
+    cudaEvent_t *ev[2] = {&s.a, &s.b};
+    for (auto e : ev) {
+      if (!c->event_pool.empty()) { *e = c->event_pool.back(); c->event_pool.pop_back(); }
+      else if (cudaEventCreate(e) != cudaSuccess) return;
+    }
+    cudaEventRecord(s.a, st);
+    c->spans.push_back(s);
+    idx = (int)c->spans.size() - 1;
+#endif
+  }
+  ~Timed() {
+#ifndef ERF_HOSTCHECK
+    if (idx >= 0) cudaEventRecord(c->spans[idx].b, st);
+#endif
+  }
+};
 
 // general path (k_general.cu)
 void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st);  // fills c->R, theta_t, pi_t

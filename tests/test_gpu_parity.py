@@ -1,0 +1,288 @@
+"""Parity of the CUDA path (through the C-ABI) with the CPU oracle, element by element on the
+same seeded inputs.  Tolerances (BASELINE.json north_star): max relative field error
+<= 1e-11 after one RK3 step, <= 1e-9 after 100 steps, fp64; error norm = DESIGN.md G24."""
+import numpy as np
+import pytest
+
+from paper_2412_04395_b200 import workloads as wl
+from util import field_errors, uniform_case
+
+pytestmark = pytest.mark.gpu
+
+TOL_1STEP = 1e-11
+TOL_100STEP = 1e-9
+TOL_RHS = 1e-11  # one operator evaluation, relative to the field maximum
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def erfo():
+    from oracle import erfo
+    erfo.build()
+    return erfo
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2412_04395_b200 import binding, build
+    build.build()
+    binding.load()
+    return binding
+
+
+def _dev(torch, arrs):
+    return [torch.as_tensor(np.ascontiguousarray(a)).cuda() for a in arrs]
+
+
+def _host(ts):
+    return [t.cpu().numpy() for t in ts]
+
+
+def _run_gpu(torch, B, case, steps, path=None, state=None):
+    d = B.Dycore(case)
+    if path is not None:
+        d.set_path(path)
+    d.set_state(*_dev(torch, state if state is not None else case["state"]))
+    for _ in range(steps):
+        d.rk3_step(case["dt"], case["ns"])
+    out = _host(d.get_state())
+    torch.cuda.synchronize()
+    n = d.launch_count
+    d.close()
+    assert n > 0
+    return out
+
+
+def _run_oracle(erfo, case, steps, state=None):
+    o = erfo.Oracle(case)
+    o.set_state(*(state if state is not None else case["state"]))
+    for _ in range(steps):
+        o.step(case["dt"], case["ns"])
+    out = o.get_state()
+    o.close()
+    return out
+
+
+SMALL = [  # several tiles plus a ragged tail in every direction
+    (1, dict(nx=40, ny=23, nz=19)),
+    (2, dict(nx=37, ny=18, nz=21)),
+    (3, dict(nx=45, ny=20, nz=34)),
+    (4, dict(nx=44, ny=36, nz=96)),
+    (5, dict(nx=70, ny=11, nz=40)),
+]
+PATHS = [0, 1]  # ERF_PATH_AUTO (fused kernels where they apply), ERF_PATH_GENERAL
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("cfg,kw", SMALL)
+def test_slow_rhs_matches_oracle(torch, erfo, B, cfg, kw, path):
+    """f(S) of Eq. 1-3 (advection Eq. 17-21, diffusion Eq. 9, pressure gradient, buoyancy)."""
+    case = wl.make_case(cfg, **kw)
+    # one oracle step first so that w, rho', p' are all non-trivial
+    st = _run_oracle(erfo, case, 1)
+    o = erfo.Oracle(case)
+    o.set_state(*st)
+    ref = o.slow_rhs()
+    d = B.Dycore(case)
+    d.set_path(path)
+    d.set_state(*_dev(torch, st))
+    got = _host(d.slow_rhs())
+    d.close()
+    for f, (a, b) in enumerate(zip(got, ref)):
+        scale = max(np.abs(b).max(), 1e-300)
+        assert np.abs(a - b).max() / scale <= TOL_RHS, (f, np.abs(a - b).max() / scale)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("cfg,kw", SMALL)
+def test_acoustic_substeps_match_oracle(torch, erfo, B, cfg, kw, path):
+    """Appendix A substeps about the current state, from a seeded perturbation."""
+    case = wl.make_case(cfg, **kw)
+    nx, ny, nz = case["nx"], case["ny"], case["nz"]
+    rng = np.random.default_rng(77 + cfg)
+    o = erfo.Oracle(case)
+    o.set_state(*case["state"])
+    R = o.slow_rhs()
+    P = [1e-3 * rng.standard_normal((nz + (f == 3), ny, nx)) for f in range(5)]
+    P[3][0] = 0.0
+    P[3][nz] = 0.0
+    dtau = case["dt"] / case["ns"]
+    ref = o.acoustic(dtau, 3, R, P)
+    d = B.Dycore(case)
+    d.set_path(path)
+    d.set_state(*_dev(torch, case["state"]))
+    got = _host(d.acoustic(dtau, 3, _dev(torch, R), _dev(torch, P)))
+    d.close()
+    # the lids of W'' are not part of the substep's result (the stage finish imposes them)
+    got[3][0] = ref[3][0]
+    got[3][nz] = ref[3][nz]
+    assert max(field_errors(got, ref)) <= TOL_1STEP, field_errors(got, ref)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("cfg,kw", SMALL)
+def test_one_step_small(torch, erfo, B, cfg, kw, path):
+    case = wl.make_case(cfg, **kw)
+    ref = _run_oracle(erfo, case, 1)
+    got = _run_gpu(torch, B, case, 1, path)
+    assert max(field_errors(got, ref)) <= TOL_1STEP, field_errors(got, ref)
+
+
+def test_config1_full(torch, erfo, B):
+    """BASELINE config 1 exactly as stated: 32^3, one step."""
+    case = wl.make_case(1)
+    ref = _run_oracle(erfo, case, case["steps"])
+    got = _run_gpu(torch, B, case, case["steps"])
+    assert max(field_errors(got, ref)) <= TOL_1STEP, field_errors(got, ref)
+
+
+def test_config2_full_size_two_steps(torch, erfo, B):
+    case = wl.make_case(2)
+    ref = _run_oracle(erfo, case, 2)
+    got = _run_gpu(torch, B, case, 2)
+    assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
+
+
+@pytest.mark.parametrize("cfg,kw,steps", [
+    (2, dict(nx=32, ny=32, nz=64), 20),
+    (3, dict(nx=32, ny=24, nz=128), 100),
+    (4, dict(nx=40, ny=32, nz=96), 50),
+    (5, dict(nx=32, ny=32, nz=128), 20),
+])
+def test_full_step_count_on_crop(torch, erfo, B, cfg, kw, steps):
+    """The configuration's own step count on a periodic crop (same spacing, dt, seed recipe)."""
+    case = wl.make_case(cfg, **kw)
+    assert steps == case["steps"]
+    ref = _run_oracle(erfo, case, steps)
+    got = _run_gpu(torch, B, case, steps)
+    tol = TOL_1STEP * steps if steps < 100 else TOL_100STEP
+    assert max(field_errors(got, ref)) <= min(tol, TOL_100STEP), field_errors(got, ref)
+
+
+# domain of dependence of one RK3 step in cells: 3 slow evaluations (advection +-3, plus the
+# Smagorinsky/stress stencil) and 1 + ns/2 + ns substeps of +-1 each
+def _margin(ns):
+    return 3 * 5 + (1 + ns // 2 + ns) + 2
+
+
+@pytest.mark.parametrize("cfg", [3, 4, 5])
+def test_full_size_sampled_windows(torch, erfo, B, cfg):
+    """BASELINE configs 3-5 at full size, in the launch configuration bench.py times: after one
+    step, sampled column windows are compared with the oracle run on the window alone (the
+    window's interior is outside the domain of dependence of its own periodic closure)."""
+    case = wl.make_case(cfg)
+    got = _run_gpu(torch, B, case, 1)
+    nx, ny = case["nx"], case["ny"]
+    mg = _margin(case["ns"])
+    w = 2 * mg + 12
+    spots = [(0, 0), (nx - w // 2, ny - w // 2)]  # one window wraps around the periodic seam
+    if cfg == 4:
+        spots = [(nx // 2 - w // 2, ny // 2 - w // 2), (nx // 2 - 4, ny // 2 - w + 6)]  # over the hill
+    for (i0, j0) in spots:
+        sub = wl.window(case, i0, j0, w, w)
+        ref = _run_oracle(erfo, sub, 1)
+        gw = wl.window(case, i0, j0, w, w, state=got)["state"]
+        inner = [a[:, mg:-mg, mg:-mg] for a in gw]
+        rin = [a[:, mg:-mg, mg:-mg] for a in ref]
+        assert max(field_errors(inner, rin)) <= TOL_1STEP, (i0, j0, field_errors(inner, rin))
+    # properties that hold at any size: mass and rho*theta are conserved (flux form)
+    if case.get("z_nodes") is None:
+        hc = np.diff(case["z_levels"])[:, None, None]
+        for f in (0, 4):
+            m0 = float((case["state"][f] * hc).sum(dtype=np.longdouble))
+            m1 = float((got[f] * hc).sum(dtype=np.longdouble))
+            assert abs(m1 - m0) <= 1e-12 * abs(m0)
+
+
+def test_general_and_fused_paths_agree_at_full_size(torch, B):
+    """On-device cross-check at BASELINE config 2's full size, 3 steps."""
+    case = wl.make_case(2)
+    a = _run_gpu(torch, B, case, 3, path=0)
+    b = _run_gpu(torch, B, case, 3, path=1)
+    assert max(field_errors(a, b)) <= 3 * TOL_1STEP
+
+
+def test_set_get_roundtrip_is_bitwise(torch, B):
+    case = wl.make_case(2, nx=24, ny=20, nz=16)
+    d = B.Dycore(case)
+    st = _dev(torch, case["state"])
+    d.set_state(*st)
+    out = _host(d.get_state())
+    d.close()
+    for f, (a, b) in enumerate(zip(out, case["state"])):
+        assert np.array_equal(a, b), f  # flat grid: the kinematic lid value of rho*w is 0
+
+
+def test_rest_state_stays_at_rest_on_gpu(torch, B):
+    """with the base state and zero wind, f(S) = 0 exactly."""
+    case = wl.make_case(3, nx=32, ny=16, nz=40)
+    nz, ny, nx = case["nz"], case["ny"], case["nx"]
+    r0 = np.broadcast_to(case["rho0"][:, None, None], (nz, ny, nx))
+    t0 = np.broadcast_to(case["rhotheta0"][:, None, None], (nz, ny, nx))
+    z = np.zeros((nz, ny, nx))
+    st = [np.array(r0), z, z.copy(), np.zeros((nz + 1, ny, nx)), np.array(t0)]
+    got = _run_gpu(torch, B, case, 3, state=st)
+    for a, b in zip(got, st):
+        assert np.array_equal(a, b)
+
+
+@pytest.mark.parametrize("kw", [dict(nx=1, ny=1, nz=8), dict(nx=5, ny=1, nz=9), dict(nx=2, ny=3, nz=2),
+                                dict(nx=33, ny=7, nz=1)])
+def test_degenerate_sizes(torch, erfo, B, kw):
+    """Single column, 2-D slab, two levels, one level: the smallest grids the method admits."""
+    case = wl.make_case(1, **kw)
+    if kw["nz"] == 1:
+        case["params"]["substep_mode"] = 0
+    ref = _run_oracle(erfo, case, 2)
+    got = _run_gpu(torch, B, case, 2)
+    assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
+
+
+@pytest.mark.parametrize("order", [2, 3, 4, 5, 6])
+def test_every_advection_order(torch, erfo, B, order):
+    case = wl.make_case(2, nx=20, ny=12, nz=14, params=dict(adv_order_h=order, adv_order_v=order))
+    ref = _run_oracle(erfo, case, 1)
+    got = _run_gpu(torch, B, case, 1)
+    assert max(field_errors(got, ref)) <= TOL_1STEP, field_errors(got, ref)
+
+
+def test_mixed_orders_and_no_substepping(torch, erfo, B):
+    case = wl.make_case(5, nx=24, ny=12, nz=16, params=dict(adv_order_h=5, adv_order_v=3, substep_mode=0))
+    case["dt"] = 0.005
+    ref = _run_oracle(erfo, case, 2)
+    got = _run_gpu(torch, B, case, 2)
+    assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
+
+
+def test_argument_errors_on_gpu(torch, B):
+    case = wl.make_case(1, nx=8, ny=8, nz=8)
+    d = B.Dycore(case)
+    d.set_state(*_dev(torch, case["state"]))
+    for dt, ns in [(0.5, 5), (0.5, 0), (0.0, 6), (-1.0, 6)]:
+        with pytest.raises(B.ErfError) as e:
+            d.rk3_step(dt, ns)
+        assert e.value.code == B.ERF_EINVAL
+    d.rk3_step(0.5, 2)  # still usable
+    d.close()
+
+
+def test_uses_the_caller_stream(torch, erfo, B):
+    case = wl.make_case(1, nx=16, ny=16, nz=12)
+    ref = _run_oracle(erfo, case, 2)
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        d = B.Dycore(case)
+        d.set_state(*_dev(torch, case["state"]))
+        d.rk3_step(case["dt"], case["ns"])
+        d.rk3_step(case["dt"], case["ns"])
+        out = d.get_state()
+    s.synchronize()
+    got = _host(out)
+    d.close()
+    assert max(field_errors(got, ref)) <= 2 * TOL_1STEP

@@ -33,3 +33,15 @@ def base_state_fields(case):
 def rel_err(a, b, scale=None):
     s = scale if scale is not None else max(np.abs(b).max(), 1e-300)
     return float(np.abs(a - b).max() / s)
+
+
+def field_errors(got, ref):
+    """Max relative field error per field (reading G24): |got-ref|_max / scale with
+    scale_rho = max|rho|, scale_Theta = max|Theta| and ONE shared scale max(|U|,|V|,|W|) for the
+    three momenta.  Order (rho, U, V, W, Theta)."""
+    got = [np.asarray(a) for a in got]
+    ref = [np.asarray(a) for a in ref]
+    tiny = 1e-300
+    sm = max(max(float(np.abs(ref[f]).max()) for f in (1, 2, 3)), tiny)
+    scale = [max(float(np.abs(ref[0]).max()), tiny), sm, sm, sm, max(float(np.abs(ref[4]).max()), tiny)]
+    return [float(np.abs(got[f] - ref[f]).max() / scale[f]) for f in range(5)]
