@@ -85,6 +85,7 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   c->diff_alloc = false;
   c->zl_dev = nullptr;
   c->timing = false;
+  c->fz = nullptr;
   for (int i = 0; i < ERF_TIMING_CLASSES; i++) { c->t_calls[i] = 0; c->t_ms[i] = 0.0; }
   memset(&c->diff, 0, sizeof(c->diff));
   memset(&c->ac, 0, sizeof(c->ac));

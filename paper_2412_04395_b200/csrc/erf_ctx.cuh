@@ -14,6 +14,8 @@ struct F5 {
   double *f[5];
 };
 
+struct FusedState;  // fused.cuh
+
 }  // namespace erfb
 
 struct erf_ctx {
@@ -39,6 +41,7 @@ struct erf_ctx {
   erfb::gen::Diff diff;
   bool diff_alloc;
   erfb::gen::Acou ac;
+  erfb::FusedState *fz;  // fused flat-grid path (null until fused_setup)
 
   // per-kernel timing (erf_set_timing)
   bool timing;

@@ -1,16 +1,46 @@
-// fused.cuh -- interface of the fused flat-grid kernels (k_fused_*.cu).
+// fused.cuh -- the fused flat-grid kernels (k_fused_*.cu) and their per-context state.
+//
+// "Flat" = z_nodes == NULL (level heights depend on k only) with a 1-D base state: every
+// metric term is a per-level constant (hx = hy = hc = dz(k), slopes = 0, Omega = W), so
+// the column operators read short per-level tables instead of 3-D metric fields.
 #pragma once
 #include "erf_ctx.cuh"
 
 namespace erfb {
 
-// allocate / precompute what the fused kernels need; called at the end of erf_create
+// per-level tables (device, length nz+1 each)
+struct LevelTables {
+  const double *dz;     // [k] cell thickness hc(k), k < nz
+  const double *rdz;    // [k] 1/hc(k)
+  const double *rhw;    // [k] 1/hw(k), k = 1..nz-1 (centre-to-centre spacing)
+  const double *tabB;   // [k] rho0f(k) * (Rd/cv) / pi0f(k) at w-face k = 1..nz-1
+  const double *rho0;   // [k] base-state density
+  const double *Th0;    // [k] base-state rho*theta
+  const double *rTh0;   // [k] 1/Th0
+  const double *p0;     // [k] base-state pressure (Eq. 7)
+};
+
+struct FusedState {
+  bool ok;            // fused kernels cover this context
+  LevelTables tab;
+  double *iT;         // 1/Theta^t (stage constant)
+  double *U2, *V2;    // second buffers of U'', V'' (ping-pong across substeps)
+  double *Thd[2];     // Theta''_d ping-pong
+  double *cp_scr;     // Thomas c' scratch when it does not fit in shared memory
+  double *mut;        // Smagorinsky eddy viscosity (cell centres)
+  int variant;        // tuning knob (erf_set_option)
+};
+
 int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st);
 void fused_release(erf_ctx *c);
-// true when the fused kernels cover this context's grid and parameters
 bool fused_available(const erf_ctx *c);
 void fused_rk3_step(erf_ctx *c, double dt, int n_acoustic, cudaStream_t st);
 void fused_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st);
 void fused_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st);
+
+// k_fused_acoustic.cu
+void launch_acoustic_flat(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st);
+// k_fused_slow.cu
+void launch_slow_flat(erf_ctx *c, const F5 &S, cudaStream_t st);
 
 }  // namespace erfb
