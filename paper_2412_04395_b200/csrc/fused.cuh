@@ -18,6 +18,8 @@ struct LevelTables {
   const double *Th0;    // [k] base-state rho*theta
   const double *rTh0;   // [k] 1/Th0
   const double *p0;     // [k] base-state pressure (Eq. 7)
+  const double *pi0;    // [k] base-state Exner function
+  const double *csd2;   // [k] (Cs Delta)^2, Delta = (dx dy dz_k)^(1/3)  [R:G9]
 };
 
 struct FusedState {
@@ -27,7 +29,7 @@ struct FusedState {
   double *U2, *V2;    // second buffers of U'', V'' (ping-pong across substeps)
   double *Thd[2];     // Theta''_d ping-pong
   double *cp_scr;     // Thomas c' scratch when it does not fit in shared memory
-  double *mut;        // Smagorinsky eddy viscosity (cell centres)
+  double *mu, *Kd;    // dynamic viscosity and scalar diffusivity at cell centres (diffusion != 0)
   int variant;        // tuning knob (erf_set_option)
 };
 

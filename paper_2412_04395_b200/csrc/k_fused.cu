@@ -8,7 +8,7 @@ namespace erfb {
 
 // per-level tables from column (0,0) of the 3-D geometry / base-state fields
 __global__ void k_level_tables(View v, double *dz, double *rdz, double *rhw, double *tabB, double *rho0,
-                               double *Th0, double *rTh0, double *p0) {
+                               double *Th0, double *rTh0, double *p0, double *pi0, double *csd2) {
   int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k > v.nz) return;
   size_t a = (size_t)k * v.ny * v.nx;
@@ -19,8 +19,11 @@ __global__ void k_level_tables(View v, double *dz, double *rdz, double *rhw, dou
     Th0[k] = v.Th0[a];
     rTh0[k] = 1.0 / v.Th0[a];
     p0[k] = v.p0[a];
+    pi0[k] = v.pi0[a];
+    const double cd = v.Cs * cbrt(v.dx * v.dy * v.hc[a]);
+    csd2[k] = cd * cd;
   } else {
-    dz[k] = rdz[k] = rho0[k] = Th0[k] = rTh0[k] = p0[k] = 0.0;
+    dz[k] = rdz[k] = rho0[k] = Th0[k] = rTh0[k] = p0[k] = pi0[k] = csd2[k] = 0.0;
   }
   if (k >= 1 && k < v.nz) {
     size_t b = (size_t)(k - 1) * v.ny * v.nx;
@@ -42,22 +45,24 @@ int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
   if (const char *e = getenv("ERF_B200_VARIANT")) z->variant = atoi(e);  // developer tuning knob
   if (!z->ok) return ERF_OK;
   const int nl = c->nz + 1;
-  double *t[8];
+  double *t[10];
   for (auto &p : t) {
     p = c->alloc(nl);
     if (!p) return c->status;
   }
-  k_level_tables<<<(nl + 127) / 128, 128, 0, st>>>(c->v, t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7]);
+  k_level_tables<<<(nl + 127) / 128, 128, 0, st>>>(c->v, t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7],
+                                                       t[8], t[9]);
   c->launches++;
-  z->tab = LevelTables{t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7]};
+  z->tab = LevelTables{t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7], t[8], t[9]};
   double **arr[] = {&z->iT, &z->U2, &z->V2, &z->Thd[0], &z->Thd[1], &z->cp_scr};
   for (auto p : arr) {
     *p = c->alloc(c->NW);
     if (!*p) return c->status;
   }
-  if (c->p.diffusion == 2) {
-    z->mut = c->alloc(c->NW);
-    if (!z->mut) return c->status;
+  if (c->p.diffusion != 0) {
+    z->mu = c->alloc(c->NW);
+    z->Kd = c->alloc(c->NW);
+    if (!z->mu || !z->Kd) return c->status;
   }
   return ERF_OK;
 }
