@@ -11,21 +11,9 @@
 // neighbours are read through L1 (a warp's shifted 256-B rows share lines).
 // On a flat grid all metric terms are per-level constants (tables), Omega = W, and every
 // horizontal slope term of D0 vanishes identically.
-#include "fused.cuh"
+#include "slow_flat.cuh"
 
 namespace erfb {
-
-struct SlowFlat {
-  int nx, ny, nz, ov;
-  double rdx, rdy, g;
-  const double *rho, *U, *V, *W, *Th;
-  double *theta, *u, *v, *w, *pp, *pi, *iT;
-  double *Rrho, *RU, *RV, *RW, *RTh;
-  double *mu, *K;
-  const double *dz, *rdz, *rhw, *rho0, *Th0, *rTh0, *p0, *pi0, *csd2;
-  double gam, rdocv, nu, alpha, rPrt;
-  int diffusion;
-};
 
 // ------------------------------------------------------------------ primitives
 __global__ void __launch_bounds__(256) k_prim_flat(const SlowFlat p) {
@@ -113,40 +101,6 @@ __global__ void __launch_bounds__(256) k_visc_flat(const SlowFlat p) {
   }
   p.mu[a] = mu;
   p.K[a] = K;
-}
-
-// ------------------------------------------------------------------ Eq. 17-21
-// q0..q5 = q_{m-3} .. q_{m+2}, flux point m-1/2; returns M * q_interp with the upwind sign of M:
-// flux = M q_even - |M| q_odd  (Eq. 20-21 with sgn = sign(M); Eq. 21 repaired [R:G1])
-template <int ORD>
-__device__ __forceinline__ double flux_c(double M, double q0, double q1, double q2, double q3, double q4, double q5) {
-  const double s2 = q3 + q2;
-  if (ORD == 2) return M * (0.5 * s2);
-  const double s4 = q4 + q1;
-  const double q4th = (7.0 / 12.0) * s2 - (1.0 / 12.0) * s4;
-  if (ORD == 4) return M * q4th;
-  if (ORD == 3) return M * q4th + fabs(M) * ((1.0 / 12.0) * ((q4 - q1) - 3.0 * (q3 - q2)));
-  const double q6th = (37.0 / 60.0) * s2 - (2.0 / 15.0) * s4 + (1.0 / 60.0) * (q5 + q0);
-  if (ORD == 6) return M * q6th;
-  return M * q6th - fabs(M) * ((1.0 / 60.0) * ((q5 - q0) - 5.0 * (q4 - q1) + 10.0 * (q3 - q2)));
-}
-
-__device__ __forceinline__ double flux_rt(int ord, double M, const double *q) {
-  switch (ord) {
-    case 2: return flux_c<2>(M, q[0], q[1], q[2], q[3], q[4], q[5]);
-    case 3: return flux_c<3>(M, q[0], q[1], q[2], q[3], q[4], q[5]);
-    case 4: return flux_c<4>(M, q[0], q[1], q[2], q[3], q[4], q[5]);
-    case 5: return flux_c<5>(M, q[0], q[1], q[2], q[3], q[4], q[5]);
-    default: return flux_c<6>(M, q[0], q[1], q[2], q[3], q[4], q[5]);
-  }
-}
-
-// order next to the lids [R:G13]; r = min(#valid points below, above)
-__device__ __forceinline__ int vorder(int req, int r) {
-  const int need = (req + 1) >> 1;
-  if (r >= need) return req;
-  if (r >= 2 && req >= 3) return (req & 1) ? 3 : 4;
-  return 2;
 }
 
 // ------------------------------------------------------------------ advection + PG + buoyancy
@@ -423,19 +377,29 @@ void launch_slow_flat(erf_ctx *c, const F5 &S, cudaStream_t st) {
   const size_t plane = (size_t)c->nx * c->ny;
   k_prim_flat<<<(unsigned)((plane * (c->nz + 1) + 255) / 256), 256, 0, st>>>(p);
   c->launches++;
+  const bool tiled = !(z->variant & 8);  // variant bit 8 (developer knob): the first, untiled column kernels
   dim3 block(32, 4), grid((c->nx + 31) / 32, (c->ny + 3) / 4);
-  switch (c->p.adv_order_h) {
-    case 2: launch_adv<2>(p, grid, block, st); break;
-    case 3: launch_adv<3>(p, grid, block, st); break;
-    case 4: launch_adv<4>(p, grid, block, st); break;
-    case 5: launch_adv<5>(p, grid, block, st); break;
-    default: launch_adv<6>(p, grid, block, st); break;
+  if (tiled) {
+    launch_adv_diff_tiled(c, p, st);
+  } else {
+    switch (c->p.adv_order_h) {
+      case 2: launch_adv<2>(p, grid, block, st); break;
+      case 3: launch_adv<3>(p, grid, block, st); break;
+      case 4: launch_adv<4>(p, grid, block, st); break;
+      case 5: launch_adv<5>(p, grid, block, st); break;
+      default: launch_adv<6>(p, grid, block, st); break;
+    }
+    c->launches++;
   }
-  c->launches++;
   if (c->p.diffusion != 0) {
     k_visc_flat<<<(unsigned)((plane * c->nz + 255) / 256), 256, 0, st>>>(p);
-    k_diff_flat<<<grid, block, 0, st>>>(p);
-    c->launches += 2;
+    c->launches++;
+    if (tiled) {
+      launch_diff_tiled(c, p, st);
+    } else {
+      k_diff_flat<<<grid, block, 0, st>>>(p);
+      c->launches++;
+    }
   }
 }
 
