@@ -105,6 +105,10 @@ __global__ void k_stage_finish_flat(size_t nc, size_t nw, size_t plane, F5 St, F
 void fused_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st) { launch_slow_flat(c, S, st); }
 
 void fused_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st) {
+  if (acoustic_zc_available(c)) {
+    launch_acoustic_zc(c, dtau, n, 0, st);
+    return;
+  }
   // entry for erf_acoustic: Theta''_prev = Theta'' => Theta''_d = Theta''
   cudaMemcpyAsync(c->fz->Thd[0], c->P.f[TH], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
   launch_acoustic_flat(c, St, dtau, n, st);
@@ -113,12 +117,21 @@ void fused_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t s
 void fused_rk3_step(erf_ctx *c, double dt, int ns, cudaStream_t st) {
   const size_t plane = (size_t)c->nx * c->ny, nc = plane * c->nz, nw = c->NW;
   const unsigned blocks = (unsigned)((nw + 255) / 256);
-  for (int f = 0; f < 5; f++)  // S^t = S^n
-    cudaMemcpyAsync(c->St.f[f], c->S.f[f], nw * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  const bool zc = acoustic_zc_available(c);
+  if (!zc)
+    for (int f = 0; f < 5; f++)  // S^t = S^n
+      cudaMemcpyAsync(c->St.f[f], c->S.f[f], nw * sizeof(double), cudaMemcpyDeviceToDevice, st);
   for (int stage = 1; stage <= 3; stage++) {
     int nsub = stage == 1 ? 1 : (stage == 2 ? ns / 2 : ns);  // L170
     double dtau = stage == 1 ? dt / 3.0 : dt / ns;
-    launch_slow_flat(c, c->St, st);  // f(S^t) every stage (L140); also theta^t, pi^t, 1/Theta^t
+    if (zc) {
+      // f(S^t) every stage (L140), S^t = S^n in stage 1; the substep kernels form S'' = S^n - S^t at their first
+      // launch and write S^t + S'' at their last (L581, L593)
+      launch_slow_flat(c, stage == 1 ? c->S : c->St, st);
+      launch_acoustic_zc(c, dtau, nsub, stage, st);
+      continue;
+    }
+    launch_slow_flat(c, c->St, st);  // also theta^t, pi^t, 1/Theta^t
     {
       Timed t(c, T_OTHER, st);
       k_stage_init_flat<<<blocks, 256, 0, st>>>(nc, nw, c->S, c->St, c->P, c->fz->Thd[0]);
