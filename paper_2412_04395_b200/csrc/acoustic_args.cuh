@@ -1,0 +1,27 @@
+// acoustic_args.cuh -- the argument block shared by the two flat-grid acoustic-substep kernels
+// (k_fused_acoustic.cu: thread per column; k_acoustic_zc.cu: z-chunked) and their common driver.
+#pragma once
+#include "fused.cuh"
+
+namespace erfb {
+
+// stage-combine bits of a substep launch
+enum { MODE_FIRST = 1, MODE_LAST = 2, MODE_ZERO = 4 };
+
+struct AcArgs {
+  int nx, ny, nz, M, ZC;
+  double dtau, rdx, rdy, b1, b2, beta_d, g, gR;
+  const double *Pu, *Pv, *Pw, *Pr, *Pt, *Ptp;  // S'' in: U'', V'', W'', rho'', Theta'' and Theta''_prev
+  const double *Sn[5], *St[5];                 // FIRST: S'' = Sn - St;  LAST: St is added to the result
+  double *oU, *oV, *oW, *oR, *oT, *oTp;        // out: S'' (or the stage result); oTp: initial Theta'' (FIRST)
+  double *kW, *kR, *kT, *cp_scr;               // column scratch between the sweeps (thread-per-column kernel)
+  const double *RU, *RV, *RW, *Rrho, *RTh;
+  const double *theta, *pi, *iT;
+  const double *rdz, *rhw, *tabB;
+};
+
+void launch_acoustic_flat_one(const AcArgs &p, int mode, cudaStream_t st);  // k_fused_acoustic.cu
+bool acoustic_zc_selected(const erf_ctx *c);                                // k_acoustic_zc.cu
+void launch_acoustic_zc_one(const erf_ctx *c, AcArgs &p, int mode, cudaStream_t st);
+
+}  // namespace erfb

@@ -40,11 +40,6 @@ void fused_rk3_step(erf_ctx *c, double dt, int n_acoustic, cudaStream_t st);
 void fused_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st);
 void fused_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st);
 
-// k_fused_acoustic.cu
-void launch_acoustic_flat(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st);
-// k_acoustic_zc.cu: z-chunked substep kernel with the stage combine folded in
-bool acoustic_zc_available(const erf_ctx *c);
-void launch_acoustic_zc(erf_ctx *c, double dtau, int n, int stage, cudaStream_t st);
 // k_fused_slow.cu
 void launch_slow_flat(erf_ctx *c, const F5 &S, cudaStream_t st);
 

@@ -28,25 +28,12 @@
 //
 // Stage combine.  MODE_FIRST: S'' = S^n - S^t is formed at load time (L581) [R:G7] (MODE_ZERO: RK stage 1,
 // S'' = 0, nothing is loaded).  MODE_LAST: the kernel writes S^t + S'' (L593) and the flat lids W = 0.
-#include "fused.cuh"
+#include "acoustic_args.cuh"
 
 namespace erfb {
 
-enum { MODE_FIRST = 1, MODE_LAST = 2, MODE_ZERO = 4 };
-
-struct AcZc {
-  int nx, ny, nz, M, ZC;
-  double dtau, rdx, rdy, b1, b2, beta_d, g, gR;
-  const double *Pu, *Pv, *Pw, *Pr, *Pt, *Ptp;  // S'' in: U'', V'', W'', rho'', Theta'' and Theta''_prev
-  const double *Sn[5], *St[5];                 // FIRST: S'' = Sn - St;  LAST: St is added to the result
-  double *oU, *oV, *oW, *oR, *oT, *oTp;        // out: S'' (or the stage result); oTp: initial Theta'' (FIRST)
-  const double *RU, *RV, *RW, *Rrho, *RTh;
-  const double *theta, *pi, *iT;
-  const double *rdz, *rhw, *tabB;
-};
-
 template <int CW, int MODE>
-__global__ void __launch_bounds__(512, 1) k_acoustic_zc(const AcZc p) {
+__global__ void __launch_bounds__(512, 1) k_acoustic_zc(const AcArgs p) {
   constexpr bool FIRST = (MODE & MODE_FIRST) != 0, LAST = (MODE & MODE_LAST) != 0, ZERO = (MODE & MODE_ZERO) != 0;
   extern __shared__ double sm[];
   const int nx = p.nx, ny = p.ny, nz = p.nz, M = p.M, ZC = p.ZC;
@@ -101,11 +88,73 @@ __global__ void __launch_bounds__(512, 1) k_acoustic_zc(const AcZc p) {
   double y1 = 0.0, v1 = 0.0, w1 = 0.0;
 
   if (act) {
-    // ---------------- phase A ----------------
+    // ---------------- phase A1: horizontal part, levels independent ----------------
+    // explicit horizontal momenta (L585 rows 1-2) at the four faces of the column; their divergences
+    // (parked in shared memory for phase A2 together with pi^t and Theta'' of the own cell)
+#pragma unroll 1
+    for (int r = 0; r < M; r++) {
+      const int k = k0 + r;
+      if (k >= nz) break;
+      const int sa = k * CW + x;
+      const size_t kk = (size_t)k * plane;
+      const size_t a = kk + oc, axm = kk + oxm, axp = kk + oxp, aym = kk + oym, ayp = kk + oyp;
+      double Tpp, d_c, d_xm, d_xp, d_ym, d_yp, U_c, U_xp, V_c, V_yp;
+      if (ZERO) {
+        Tpp = d_c = d_xm = d_xp = d_ym = d_yp = U_c = U_xp = V_c = V_yp = 0.0;
+      } else if (FIRST) {
+        const double *__restrict__ nT = p.Sn[TH], *__restrict__ tT = p.St[TH];
+        const double n0 = nT[a], n1 = nT[axm], n2 = nT[axp], n3 = nT[aym], n4 = nT[ayp];
+        const double t0 = tT[a], t1 = tT[axm], t2 = tT[axp], t3 = tT[aym], t4 = tT[ayp];
+        const double un0 = p.Sn[UU][a], un1 = p.Sn[UU][axp], ut0 = p.St[UU][a], ut1 = p.St[UU][axp];
+        const double vn0 = p.Sn[VV][a], vn1 = p.Sn[VV][ayp], vt0 = p.St[VV][a], vt1 = p.St[VV][ayp];
+        Tpp = d_c = n0 - t0; d_xm = n1 - t1; d_xp = n2 - t2; d_ym = n3 - t3; d_yp = n4 - t4;
+        U_c = un0 - ut0; U_xp = un1 - ut1; V_c = vn0 - vt0; V_yp = vn1 - vt1;
+      } else {
+        const double *__restrict__ cT = p.Pt, *__restrict__ pT = p.Ptp;
+        const double n0 = cT[a], n1 = cT[axm], n2 = cT[axp], n3 = cT[aym], n4 = cT[ayp];
+        const double t0 = pT[a], t1 = pT[axm], t2 = pT[axp], t3 = pT[aym], t4 = pT[ayp];
+        U_c = p.Pu[a]; U_xp = p.Pu[axp]; V_c = p.Pv[a]; V_yp = p.Pv[ayp];
+        Tpp = n0;  // Theta''_d = Theta'' + beta_d (Theta'' - Theta''_prev) (L144) [R:G6]
+        d_c = n0 + beta_d * (n0 - t0); d_xm = n1 + beta_d * (n1 - t1); d_xp = n2 + beta_d * (n2 - t2);
+        d_ym = n3 + beta_d * (n3 - t3); d_yp = n4 + beta_d * (n4 - t4);
+      }
+      const double pi_c = pi[a], pi_xm = pi[axm], pi_xp = pi[axp], pi_ym = pi[aym], pi_yp = pi[ayp];
+      const double th_c = theta[a], th_xm = theta[axm], th_xp = theta[axp], th_ym = theta[aym], th_yp = theta[ayp];
+      const double ru_c = RU[a], ru_xp = RU[axp], rv_c = RV[a], rv_yp = RV[ayp];
+      double su = 0.0, sv = 0.0;
+      if (LAST) { su = p.St[UU][a]; sv = p.St[VV][a]; }
+      const double Um = U_c + dtau * ru_c - cU * (pi_xm + pi_c) * (d_c - d_xm);
+      const double Up = U_xp + dtau * ru_xp - cU * (pi_c + pi_xp) * (d_xp - d_c);
+      const double Vm = V_c + dtau * rv_c - cV * (pi_ym + pi_c) * (d_c - d_ym);
+      const double Vp = V_yp + dtau * rv_yp - cV * (pi_c + pi_yp) * (d_yp - d_c);
+      const double DhT = (Up * (th_c + th_xp) - Um * (th_xm + th_c)) * hx + (Vp * (th_c + th_yp) - Vm * (th_ym + th_c)) * hy;
+      const double Dh = (Up - Um) * p.rdx + (Vp - Vm) * p.rdy;
+      p.oU[a] = LAST ? su + Um : Um;
+      p.oV[a] = LAST ? sv + Vm : Vm;
+      if (FIRST && !LAST && !ZERO) p.oTp[a] = d_c;  // Theta''_prev of the next substep
+      TtS[sa] = DhT; rtS[sa] = Dh; cpS[sa] = pi_c; ypS[sa] = Tpp;
+    }
+    // ---------------- phase A2: vertical part, marching upward through the chunk ----------------
+    struct Lv {  // what one level needs from global memory
+      double om_t, rpp, RTh, Rrho, RW, iT, th_t, rdz, rhw, tabB;
+    };
+    auto load_lv = [&](int k, Lv &q) {
+      const int kc = min(k, nz - 1);
+      const size_t a = (size_t)kc * plane + oc;
+      const bool top = kc + 1 >= nz;
+      const size_t at = top ? a : a + plane;
+      q.om_t = pert(WW, p.Pw, at);
+      q.th_t = theta[at];
+      q.rpp = pert(RHO, p.Pr, a);
+      q.RTh = RTh[a]; q.Rrho = Rrho[a]; q.RW = RW[a]; q.iT = iTf[a];
+      q.rdz = rdz[kc]; q.rhw = rhwt[kc]; q.tabB = tabB[kc];
+    };
     double th_c = 0.0, thf_b = 0.0, om_b = 0.0;
     double pi_m = 0.0, iT_m = 0.0, rT_m = 0.0, rhc_m = 0.0, That_m = 0.0, rhat_m = 0.0, thf_bm = 0.0;
     double cp_m = 0.0, yp_m = 0.0, vp_m = 0.0;
+    Lv cur, nxt;
     if (k0 < nz) {
+      load_lv(k0, cur);
       th_c = theta[(size_t)k0 * plane + oc];
       if (k0 >= 1) {
         const size_t am = (size_t)(k0 - 1) * plane + oc;
@@ -127,45 +176,15 @@ __global__ void __launch_bounds__(512, 1) k_acoustic_zc(const AcZc p) {
         cpS[sa] = 0.0; ypS[sa] = 0.0; vpS[sa] = 0.0; TtS[sa] = 0.0; rtS[sa] = 0.0; tfS[sa] = 0.0;
         continue;
       }
-      const size_t kk = (size_t)k * plane;
-      const size_t a = kk + oc, axm = kk + oxm, axp = kk + oxp, aym = kk + oym, ayp = kk + oyp;
+      if (r + 1 < M) load_lv(k + 1, nxt);  // software pipeline: the next level's loads fly during this level's math
       const bool top = k + 1 >= nz;
-      double Tpp = 0.0, d_c = 0.0;  // Theta'' and Theta''_d of the own cell
-      if (FIRST) {
-        Tpp = d_c = thd(a);
-      } else {
-        Tpp = p.Pt[a];
-        d_c = Tpp + beta_d * (Tpp - p.Ptp[a]);
-      }
-      const double d_xm = thd(axm), d_xp = thd(axp), d_ym = thd(aym), d_yp = thd(ayp);
-      const double pi_c = pi[a], pi_xm = pi[axm], pi_xp = pi[axp], pi_ym = pi[aym], pi_yp = pi[ayp];
-      const double th_xm = theta[axm], th_xp = theta[axp], th_ym = theta[aym], th_yp = theta[ayp];
-      const double th_t = top ? 0.0 : theta[a + plane];
-      const double om_t = top ? 0.0 : pert(WW, p.Pw, a + plane);
-      const double U_c = pert(UU, p.Pu, a), U_xp = pert(UU, p.Pu, axp);
-      const double V_c = pert(VV, p.Pv, a), V_yp = pert(VV, p.Pv, ayp);
-      const double rpp = pert(RHO, p.Pr, a);
-      const double iT = iTf[a];
-      // explicit horizontal momenta (L585 rows 1-2) at the four faces of the column
-      const double Um = U_c + dtau * RU[a] - cU * (pi_xm + pi_c) * (d_c - d_xm);
-      const double Up = U_xp + dtau * RU[axp] - cU * (pi_c + pi_xp) * (d_xp - d_c);
-      const double Vm = V_c + dtau * RV[a] - cV * (pi_ym + pi_c) * (d_c - d_ym);
-      const double Vp = V_yp + dtau * RV[ayp] - cV * (pi_c + pi_yp) * (d_yp - d_c);
-      if (LAST) {
-        p.oU[a] = p.St[UU][a] + Um;
-        p.oV[a] = p.St[VV][a] + Vm;
-      } else {
-        p.oU[a] = Um;
-        p.oV[a] = Vm;
-      }
-      if (FIRST && !LAST && !ZERO) p.oTp[a] = d_c;  // Theta''_prev of the next substep
+      const double DhT = TtS[sa], Dh = rtS[sa], pi_c = cpS[sa], Tpp = ypS[sa];
+      const double om_t = top ? 0.0 : cur.om_t;
+      const double rpp = cur.rpp, iT = cur.iT, rhc = cur.rdz;
       // explicit parts of Theta'' and rho'' (L585 rows 4-5 with the old-time part of the Omega'' average)
-      const double thf_t = top ? 0.0 : 0.5 * (th_c + th_t);
-      const double rhc = rdz[k];
-      const double DhT = (Up * (th_c + th_xp) - Um * (th_xm + th_c)) * hx + (Vp * (th_c + th_yp) - Vm * (th_ym + th_c)) * hy;
-      const double Dh = (Up - Um) * p.rdx + (Vp - Vm) * p.rdy;
-      const double Ttil = Tpp + dtau * (RTh[a] - DhT - b1 * (thf_t * om_t - thf_b * om_b) * rhc);
-      const double rtil = rpp + dtau * (Rrho[a] - Dh - b1 * (om_t - om_b) * rhc);
+      const double thf_t = top ? 0.0 : 0.5 * (th_c + cur.th_t);
+      const double Ttil = Tpp + dtau * (cur.RTh - DhT - b1 * (thf_t * om_t - thf_b * om_b) * rhc);
+      const double rtil = rpp + dtau * (cur.Rrho - Dh - b1 * (om_t - om_b) * rhc);
       const double That = b2 * Ttil + b1 * Tpp, rhat = b2 * rtil + b1 * rpp;
       const double rT = rhc * iT;
       TtS[sa] = Ttil;
@@ -174,15 +193,15 @@ __global__ void __launch_bounds__(512, 1) k_acoustic_zc(const AcZc p) {
       if (k >= 1) {
         // row k of the tridiagonal system for Omega''new (S5)
         const double pif = 0.5 * (pi_m + pi_c);
-        const double rhw = rhwt[k];
-        const double Bf = tabB[k] * pif;
+        const double rhw = cur.rhw;
+        const double Bf = cur.tabB * pif;
         const double a1 = s * gR * pif * rhw, bB = sg2 * Bf;
         double Cc = thf_t * (bB * rT - a1 * rhc) - sg2 * rhc;
         double Ac = sg2 * rhc_m - thf_bm * (a1 * rhc_m + bB * rT_m);
         const double Dc = 1.0 + thf_b * (a1 * (rhc + rhc_m) - bB * (rT - rT_m)) + sg2 * (rhc - rhc_m);
         if (k == nz - 1) Cc = 0.0;
         if (k == 1) Ac = 0.0;
-        const double rw = RW[a];
+        const double rw = cur.RW;
         if (r == 0) {  // separator: That, rhat of the cell below arrive through shared memory
           sA = Ac; sC = Cc; sD = Dc; s_omb = om_b; s_RW = rw; s_c1 = gR * pif * rhw; s_c2 = g * Bf * 0.5;
           s_That = That; s_rhat = rhat; s_iT = iT; s_iTm = iT_m;
@@ -196,15 +215,14 @@ __global__ void __launch_bounds__(512, 1) k_acoustic_zc(const AcZc p) {
           vp_m = (r == 1 ? Ac : -Ac * vp_m) * minv;
           cpS[sa] = cp_m; ypS[sa] = yp_m; vpS[sa] = vp_m;
         }
-      } else if (r != 0) {
-        cpS[sa] = 0.0; ypS[sa] = 0.0; vpS[sa] = 0.0;
       }
       if (r == M - 1 || top) {
         exT[c * CW + x] = That;
         exr[c * CW + x] = rhat;
       }
-      pi_m = pi_c; th_c = th_t; thf_bm = thf_b; thf_b = thf_t; iT_m = iT; rT_m = rT; rhc_m = rhc;
+      pi_m = pi_c; th_c = cur.th_t; thf_bm = thf_b; thf_b = thf_t; iT_m = iT; rT_m = rT; rhc_m = rhc;
       That_m = That; rhat_m = rhat; om_b = om_t;
+      cur = nxt;
     }
     // interior solution at r = 1 as y1 - v1 xs_c - w1 xs_{c+1} (own shared-memory values only)
     {
@@ -314,14 +332,14 @@ static ZcGeom zc_geometry(int nz, int variant) {
   return gm;
 }
 
-bool acoustic_zc_available(const erf_ctx *c) {
-  if (!c->fz || !c->fz->ok || (c->fz->variant & 8)) return false;
+bool acoustic_zc_selected(const erf_ctx *c) {
+  if (!c->fz || !c->fz->ok || !(c->fz->variant & 32)) return false;  // developer knob: bit 32 selects this kernel
   return zc_geometry(c->nz, c->fz->variant).ok;
 }
 
 template <int CW>
-static void zc_launch(const AcZc &p, int mode, dim3 grid, int threads, size_t smem, cudaStream_t st) {
-  void (*kern)(AcZc) = nullptr;
+static void zc_launch(const AcArgs &p, int mode, dim3 grid, int threads, size_t smem, cudaStream_t st) {
+  void (*kern)(AcArgs) = nullptr;
   switch (mode) {
     case 0: kern = k_acoustic_zc<CW, 0>; break;
     case MODE_FIRST: kern = k_acoustic_zc<CW, MODE_FIRST>; break;
@@ -333,86 +351,13 @@ static void zc_launch(const AcZc &p, int mode, dim3 grid, int threads, size_t sm
   kern<<<grid, threads, smem, st>>>(p);
 }
 
-// n substeps of size dtau.  stage = 0: S'' in/out in c->P (erf_acoustic); stage = 1: RK stage 1 (S^t = S^n = c->S,
-// S'' = 0, result -> c->St); stage >= 2: S'' = c->S - c->St at the first substep, c->St += S'' at the last.
-void launch_acoustic_zc(erf_ctx *c, double dtau, int n, int stage, cudaStream_t st) {
-  FusedState *z = c->fz;
-  if (n <= 0) return;
-  const ZcGeom gm = zc_geometry(c->nz, z->variant);
-  AcZc p;
-  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.M = gm.M; p.ZC = gm.ZC;
-  p.dtau = dtau; p.rdx = 1.0 / c->v.dx; p.rdy = 1.0 / c->v.dy;
-  p.b1 = 0.5 * (1.0 - c->v.beta_s); p.b2 = 0.5 * (1.0 + c->v.beta_s);  // L589
-  p.beta_d = c->v.beta_d; p.g = c->v.g; p.gR = c->v.gam * c->v.Rd;
-  p.RU = c->R.f[UU]; p.RV = c->R.f[VV]; p.RW = c->R.f[WW]; p.Rrho = c->R.f[RHO]; p.RTh = c->R.f[TH];
-  p.theta = c->theta_t; p.pi = c->pi_t; p.iT = z->iT;
-  p.rdz = z->tab.rdz; p.rhw = z->tab.rhw; p.tabB = z->tab.tabB;
+void launch_acoustic_zc_one(const erf_ctx *c, AcArgs &p, int mode, cudaStream_t st) {
+  const ZcGeom gm = zc_geometry(c->nz, c->fz->variant);
+  p.M = gm.M; p.ZC = gm.ZC;
   dim3 grid((c->nx + gm.CW - 1) / gm.CW, c->ny);
   const int threads = gm.CW * gm.ZC;
-
-  // the three Theta'' buffers
-  double *cur = c->P.f[TH], *prev = c->P.f[TH], *fr[2] = {z->Thd[0], z->Thd[1]};
-  int nfree = 2;
-  bool rotated = false;
-  for (int sidx = 0; sidx < n; sidx++) {
-    Timed t(c, T_ACOUSTIC_FUSED, st);
-    const bool first = stage >= 1 && sidx == 0, last = stage >= 1 && sidx == n - 1;
-    int mode = (first ? MODE_FIRST : 0) | (last ? MODE_LAST : 0);
-    if (stage == 1) mode |= MODE_ZERO;
-    for (int f = 0; f < 5; f++) {
-      p.Sn[f] = c->S.f[f];
-      p.St[f] = stage == 1 ? c->S.f[f] : c->St.f[f];
-    }
-    p.Pu = c->P.f[UU]; p.Pv = c->P.f[VV]; p.Pw = c->P.f[WW]; p.Pr = c->P.f[RHO]; p.Pt = cur; p.Ptp = prev;
-    p.oTp = nullptr;
-    bool swap_uv = false, swap_stage = false;
-    if (last) {
-      if (stage == 1) {  // out of place: S^n -> S^t buffers
-        p.oU = c->St.f[UU]; p.oV = c->St.f[VV]; p.oW = c->St.f[WW]; p.oR = c->St.f[RHO]; p.oT = c->St.f[TH];
-      } else if (first) {  // neighbours still read S^t: write the stage result to the S'' buffers, then swap
-        p.oU = c->P.f[UU]; p.oV = c->P.f[VV]; p.oW = c->P.f[WW]; p.oR = c->P.f[RHO]; p.oT = c->P.f[TH];
-        swap_stage = true;
-      } else {  // in place (own cells only)
-        p.oU = c->St.f[UU]; p.oV = c->St.f[VV]; p.oW = c->St.f[WW]; p.oR = c->St.f[RHO]; p.oT = c->St.f[TH];
-      }
-    } else if (first) {
-      p.oU = c->P.f[UU]; p.oV = c->P.f[VV]; p.oW = c->P.f[WW]; p.oR = c->P.f[RHO];
-      p.oTp = c->P.f[TH];   // initial Theta'' = Theta''_prev of the next substep
-      p.oT = fr[--nfree];
-      rotated = true;
-    } else {
-      p.oU = z->U2; p.oV = z->V2; p.oW = c->P.f[WW]; p.oR = c->P.f[RHO];
-      p.oT = fr[--nfree];
-      rotated = true;
-      swap_uv = true;
-    }
-    if (gm.CW == 16) zc_launch<16>(p, mode, grid, threads, gm.smem, st);
-    else zc_launch<32>(p, mode, grid, threads, gm.smem, st);
-    c->launches++;
-    if (swap_uv) {
-      double *t1 = c->P.f[UU]; c->P.f[UU] = z->U2; z->U2 = t1;
-      double *t2 = c->P.f[VV]; c->P.f[VV] = z->V2; z->V2 = t2;
-    }
-    if (swap_stage)
-      for (int f = 0; f < 5; f++) { double *t1 = c->St.f[f]; c->St.f[f] = c->P.f[f]; c->P.f[f] = t1; }
-    if (!last) {
-      if (first) {
-        prev = c->P.f[TH];
-      } else {
-        if (prev != cur) fr[nfree++] = prev;
-        prev = cur;
-      }
-      cur = p.oT;
-    }
-  }
-  // keep three distinct Theta'' buffers: the live one in c->P
-  if (rotated && cur != c->P.f[TH]) {
-    double *others[2];
-    int m = 0;
-    if (prev != cur) others[m++] = prev;
-    for (int q = 0; q < nfree && m < 2; q++) others[m++] = fr[q];
-    c->P.f[TH] = cur; z->Thd[0] = others[0]; z->Thd[1] = others[1];
-  }
+  if (gm.CW == 16) zc_launch<16>(p, mode, grid, threads, gm.smem, st);
+  else zc_launch<32>(p, mode, grid, threads, gm.smem, st);
 }
 
 }  // namespace erfb

@@ -2,7 +2,7 @@
 #include <cstdlib>
 #include <cstring>
 
-#include "fused.cuh"
+#include "acoustic_args.cuh"
 
 namespace erfb {
 
@@ -74,75 +74,108 @@ void fused_release(erf_ctx *c) {
 
 bool fused_available(const erf_ctx *c) { return c->fz && c->fz->ok; }
 
-// S'' = S^n - S^t (L581) [R:G7]; Theta''_d = Theta'' (Theta''_prev = Theta'' at the start of a stage)
-__global__ void k_stage_init_flat(size_t nc, size_t nw, F5 S, F5 St, F5 P, double *thd) {
-  size_t a = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (a >= nw) return;
-  P.f[WW][a] = S.f[WW][a] - St.f[WW][a];
-  if (a < nc) {
-    P.f[RHO][a] = S.f[RHO][a] - St.f[RHO][a];
-    P.f[UU][a] = S.f[UU][a] - St.f[UU][a];
-    P.f[VV][a] = S.f[VV][a] - St.f[VV][a];
-    double t = S.f[TH][a] - St.f[TH][a];
-    P.f[TH][a] = t;
-    thd[a] = t;
-  }
-}
-
-// S = S^t + S'' (L593); flat lids: W = 0 at k = 0 and k = nz
-__global__ void k_stage_finish_flat(size_t nc, size_t nw, size_t plane, F5 St, F5 P) {
-  size_t a = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (a >= nw) return;
-  St.f[WW][a] = (a < plane || a >= nc) ? 0.0 : St.f[WW][a] + P.f[WW][a];
-  if (a < nc) {
-    St.f[RHO][a] += P.f[RHO][a];
-    St.f[UU][a] += P.f[UU][a];
-    St.f[VV][a] += P.f[VV][a];
-    St.f[TH][a] += P.f[TH][a];
-  }
-}
-
 void fused_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st) { launch_slow_flat(c, S, st); }
 
-void fused_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st) {
-  if (acoustic_zc_available(c)) {
-    launch_acoustic_zc(c, dtau, n, 0, st);
-    return;
+// n acoustic substeps of size dtau (Appendix A), one kernel each, with the RK stage combine folded in.
+//   stage 0: S'' in/out in c->P about the stage state c->S (erf_acoustic);
+//   stage 1: RK stage 1: S^t = S^n = c->S, S'' = 0, the stage result goes to c->St;
+//   stage 2, 3: S'' = c->S - c->St at the first substep (L581) [R:G7], c->St += S'' at the last (L593).
+// U'', V'' ping-pong between c->P and (U2, V2); Theta'' rotates through three buffers so that
+// Theta''_d = Theta'' + beta_d (Theta'' - Theta''_prev) (L144) [R:G6] can be formed at load time.
+static void acoustic_substeps(erf_ctx *c, double dtau, int n, int stage, cudaStream_t st) {
+  FusedState *z = c->fz;
+  if (n <= 0) return;
+  const bool zc = acoustic_zc_selected(c);
+  AcArgs p;
+  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.M = 0; p.ZC = 0;
+  p.dtau = dtau; p.rdx = 1.0 / c->v.dx; p.rdy = 1.0 / c->v.dy;
+  p.b1 = 0.5 * (1.0 - c->v.beta_s); p.b2 = 0.5 * (1.0 + c->v.beta_s);  // L589
+  p.beta_d = c->v.beta_d; p.g = c->v.g; p.gR = c->v.gam * c->v.Rd;
+  p.RU = c->R.f[UU]; p.RV = c->R.f[VV]; p.RW = c->R.f[WW]; p.Rrho = c->R.f[RHO]; p.RTh = c->R.f[TH];
+  p.theta = c->theta_t; p.pi = c->pi_t; p.iT = z->iT;
+  p.rdz = z->tab.rdz; p.rhw = z->tab.rhw; p.tabB = z->tab.tabB;
+  p.cp_scr = z->cp_scr;
+
+  double *cur = c->P.f[TH], *prev = c->P.f[TH], *fr[2] = {z->Thd[0], z->Thd[1]};  // the three Theta'' buffers
+  int nfree = 2;
+  bool rotated = false;
+  for (int sidx = 0; sidx < n; sidx++) {
+    Timed t(c, T_ACOUSTIC_FUSED, st);
+    const bool first = stage >= 1 && sidx == 0, last = stage >= 1 && sidx == n - 1;
+    int mode = (first ? MODE_FIRST : 0) | (last ? MODE_LAST : 0);
+    if (stage == 1) mode |= MODE_ZERO;
+    for (int f = 0; f < 5; f++) {
+      p.Sn[f] = c->S.f[f];
+      p.St[f] = stage == 1 ? c->S.f[f] : c->St.f[f];
+    }
+    p.Pu = c->P.f[UU]; p.Pv = c->P.f[VV]; p.Pw = c->P.f[WW]; p.Pr = c->P.f[RHO]; p.Pt = cur; p.Ptp = prev;
+    p.oTp = nullptr;
+    bool swap_uv = false, swap_stage = false;
+    if (last) {
+      if (stage == 1) {  // out of place: S^n -> S^t buffers
+        p.oU = c->St.f[UU]; p.oV = c->St.f[VV]; p.oW = c->St.f[WW]; p.oR = c->St.f[RHO]; p.oT = c->St.f[TH];
+      } else if (first) {  // neighbours still read S^t: write the stage result to the S'' buffers, then swap
+        p.oU = c->P.f[UU]; p.oV = c->P.f[VV]; p.oW = c->P.f[WW]; p.oR = c->P.f[RHO]; p.oT = c->P.f[TH];
+        swap_stage = true;
+      } else {  // in place (own cells only)
+        p.oU = c->St.f[UU]; p.oV = c->St.f[VV]; p.oW = c->St.f[WW]; p.oR = c->St.f[RHO]; p.oT = c->St.f[TH];
+      }
+    } else if (first) {
+      p.oU = c->P.f[UU]; p.oV = c->P.f[VV]; p.oW = c->P.f[WW]; p.oR = c->P.f[RHO];
+      p.oTp = c->P.f[TH];  // initial Theta'' = Theta''_prev of the next substep
+      p.oT = fr[--nfree];
+      rotated = true;
+    } else {
+      p.oU = z->U2; p.oV = z->V2; p.oW = c->P.f[WW]; p.oR = c->P.f[RHO];
+      p.oT = fr[--nfree];
+      rotated = true;
+      swap_uv = true;
+    }
+    // column scratch of the thread-per-column kernel: the outputs themselves, except where the output buffer
+    // still holds the stage state that is added at the end (in-place LAST): then the consumed S'' buffers
+    if (last && !first) { p.kW = c->P.f[WW]; p.kR = c->P.f[RHO]; p.kT = fr[nfree - 1]; }
+    else { p.kW = p.oW; p.kR = p.oR; p.kT = p.oT; }
+    if (zc) launch_acoustic_zc_one(c, p, mode, st);
+    else launch_acoustic_flat_one(p, mode, st);
+    c->launches++;
+    if (swap_uv) {
+      double *t1 = c->P.f[UU]; c->P.f[UU] = z->U2; z->U2 = t1;
+      double *t2 = c->P.f[VV]; c->P.f[VV] = z->V2; z->V2 = t2;
+    }
+    if (swap_stage)
+      for (int f = 0; f < 5; f++) { double *t1 = c->St.f[f]; c->St.f[f] = c->P.f[f]; c->P.f[f] = t1; }
+    if (!last) {
+      if (first) {
+        prev = c->P.f[TH];
+      } else {
+        if (prev != cur) fr[nfree++] = prev;
+        prev = cur;
+      }
+      cur = p.oT;
+    }
   }
-  // entry for erf_acoustic: Theta''_prev = Theta'' => Theta''_d = Theta''
-  cudaMemcpyAsync(c->fz->Thd[0], c->P.f[TH], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
-  launch_acoustic_flat(c, St, dtau, n, st);
+  // keep three distinct Theta'' buffers: the live one in c->P
+  if (rotated && cur != c->P.f[TH]) {
+    double *others[2];
+    int m = 0;
+    if (prev != cur) others[m++] = prev;
+    for (int q = 0; q < nfree && m < 2; q++) others[m++] = fr[q];
+    c->P.f[TH] = cur; z->Thd[0] = others[0]; z->Thd[1] = others[1];
+  }
+}
+
+void fused_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st) {
+  (void)St;
+  acoustic_substeps(c, dtau, n, 0, st);
 }
 
 void fused_rk3_step(erf_ctx *c, double dt, int ns, cudaStream_t st) {
-  const size_t plane = (size_t)c->nx * c->ny, nc = plane * c->nz, nw = c->NW;
-  const unsigned blocks = (unsigned)((nw + 255) / 256);
-  const bool zc = acoustic_zc_available(c);
-  if (!zc)
-    for (int f = 0; f < 5; f++)  // S^t = S^n
-      cudaMemcpyAsync(c->St.f[f], c->S.f[f], nw * sizeof(double), cudaMemcpyDeviceToDevice, st);
   for (int stage = 1; stage <= 3; stage++) {
     int nsub = stage == 1 ? 1 : (stage == 2 ? ns / 2 : ns);  // L170
     double dtau = stage == 1 ? dt / 3.0 : dt / ns;
-    if (zc) {
-      // f(S^t) every stage (L140), S^t = S^n in stage 1; the substep kernels form S'' = S^n - S^t at their first
-      // launch and write S^t + S'' at their last (L581, L593)
-      launch_slow_flat(c, stage == 1 ? c->S : c->St, st);
-      launch_acoustic_zc(c, dtau, nsub, stage, st);
-      continue;
-    }
-    launch_slow_flat(c, c->St, st);  // also theta^t, pi^t, 1/Theta^t
-    {
-      Timed t(c, T_OTHER, st);
-      k_stage_init_flat<<<blocks, 256, 0, st>>>(nc, nw, c->S, c->St, c->P, c->fz->Thd[0]);
-      c->launches++;
-    }
-    launch_acoustic_flat(c, c->St, dtau, nsub, st);
-    {
-      Timed t(c, T_OTHER, st);
-      k_stage_finish_flat<<<blocks, 256, 0, st>>>(nc, nw, plane, c->St, c->P);
-      c->launches++;
-    }
+    // f(S^t) every stage (L140) (also theta^t, pi^t, 1/Theta^t); S^t = S^n in stage 1
+    launch_slow_flat(c, stage == 1 ? c->S : c->St, st);
+    acoustic_substeps(c, dtau, nsub, stage, st);
   }
   for (int f = 0; f < 5; f++) {
     double *t = c->S.f[f];

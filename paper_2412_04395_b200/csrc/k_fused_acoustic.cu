@@ -10,50 +10,39 @@
 // barrier in the k loop); therefore U'', V'' and Theta''_d are double-buffered across
 // substeps (a neighbour may still need the old value after the owner has produced the new).
 //
-// Column scratch between the two sweeps (4 values per level): c' of the Thomas sweep lives in
-// shared memory when it fits (else in an HBM array), d' is parked in the W'' array, the explicit
-// parts of Theta'' and rho'' in the Theta''_d output buffer and the rho'' array -- all addresses
-// this column alone owns and rewrites in the backward sweep, so the round trip stays in L2.
+// Column scratch between the two sweeps (4 values per level): c' of the Thomas sweep in an HBM
+// array, d' parked in the W'' output, the explicit parts of Theta'' and rho'' in the Theta'' and
+// rho'' outputs -- all addresses this column alone owns and rewrites in the backward sweep.
 //
-// Algorithmic HBM traffic per cell per substep: reads U'',V'',W'',rho'',Theta'',Theta''_d, the 5
-// slow tendencies, theta^t, pi^t, 1/Theta^t (14); writes U'',V'',W'',rho'',Theta'',Theta''_d (6).
-#include "fused.cuh"
+// Theta''_d = Theta'' + beta_d (Theta'' - Theta''_prev) (L144) [R:G6] is formed at load time from the
+// current and the previous Theta'' (three rotating buffers) instead of being stored.
+//
+// Stage combine folded in (MODE bits).  FIRST: S'' = S^n - S^t is formed at load time (L581) [R:G7]
+// (ZERO: RK stage 1, S'' = 0, nothing is loaded).  LAST: the kernel writes S^t + S'' (L593) and the
+// flat lids W = 0, so no separate stage-init / stage-finish pass touches HBM.
+//
+// Algorithmic HBM traffic per cell per substep: reads U'',V'',W'',rho'',Theta'',Theta''_prev, the 5
+// slow tendencies, theta^t, pi^t, 1/Theta^t (14); writes U'',V'',W'',rho'',Theta'' (5).
+#include "acoustic_args.cuh"
 
 namespace erfb {
 
-struct AcFlat {
-  int nx, ny, nz;
-  double dtau, rdx, rdy, b1, b2, beta_d, g, gR;
-  const double *thd_in;
-  double *thd_out;
-  const double *U_in, *V_in;
-  double *U_out, *V_out;
-  double *W, *rho, *Th;
-  const double *RU, *RV, *RW, *Rrho, *RTh;
-  const double *theta, *pi, *iT;
-  const double *rdz, *rhw, *tabB;
-  double *cp_scr;
-};
-
 // everything the forward sweep reads at one level
 struct FwdIn {
-  double d_c, d_xm, d_xp, d_ym, d_yp;       // Theta''_d
+  double T_c, d_c, d_xm, d_xp, d_ym, d_yp;  // Theta'' of the own cell; Theta''_d
   double pi_c, pi_xm, pi_xp, pi_ym, pi_yp;  // pi^t
   double th_xm, th_xp, th_ym, th_yp, th_t;  // theta^t neighbours and theta^t(k+1)
   double U_c, U_xp, RU_c, RU_xp, V_c, V_yp, RV_c, RV_yp;
-  double om_t, RW, Tpp, rpp, RTh, Rrho, iT;
+  double om_t, RW, rpp, RTh, Rrho, iT, sU, sV;
 };
 
-// PF: forward-sweep software prefetch depth in levels (0 or 1); BD: backward-sweep prefetch depth;
-// MINB: blocks per SM the register allocation must allow.
-template <int ROWS, bool CP_SMEM, int PF, int MINB>
-__global__ void __launch_bounds__(32 * ROWS, MINB) k_acoustic_flat(const AcFlat p) {
+template <int ROWS, int MODE>
+__global__ void __launch_bounds__(32 * ROWS, 4) k_acoustic_flat(const AcArgs p) {
+  constexpr bool FIRST = (MODE & MODE_FIRST) != 0, LAST = (MODE & MODE_LAST) != 0, ZERO = (MODE & MODE_ZERO) != 0;
   constexpr int BD = 4;
-  extern __shared__ double s_cp[];  // [nz][32*ROWS] when CP_SMEM
   const int lane = threadIdx.x, row = threadIdx.y;
   const int i = blockIdx.x * 32 + lane, j = blockIdx.y * ROWS + row;
   if (i >= p.nx || j >= p.ny) return;
-  const int tid = row * 32 + lane, nthr = 32 * ROWS;
   const int nx = p.nx, ny = p.ny, nz = p.nz;
   const int im = i == 0 ? nx - 1 : i - 1, ip = i == nx - 1 ? 0 : i + 1;
   const int jm = j == 0 ? ny - 1 : j - 1, jp = j == ny - 1 ? 0 : j + 1;
@@ -61,35 +50,51 @@ __global__ void __launch_bounds__(32 * ROWS, MINB) k_acoustic_flat(const AcFlat 
   const size_t oc = (size_t)j * nx + i, oxm = (size_t)j * nx + im, oxp = (size_t)j * nx + ip;
   const size_t oym = (size_t)jm * nx + i, oyp = (size_t)jp * nx + i;
 
-  const double *__restrict__ thd_in = p.thd_in;
-  double *__restrict__ thd_out = p.thd_out;
-  const double *__restrict__ U_in = p.U_in, *__restrict__ V_in = p.V_in;
-  double *__restrict__ U_out = p.U_out, *__restrict__ V_out = p.V_out;
-  double *__restrict__ Wf = p.W, *__restrict__ rhof = p.rho, *__restrict__ Thf = p.Th;
   const double *__restrict__ RU = p.RU, *__restrict__ RV = p.RV, *__restrict__ RW = p.RW;
   const double *__restrict__ Rrho = p.Rrho, *__restrict__ RTh = p.RTh;
   const double *__restrict__ theta = p.theta, *__restrict__ pi = p.pi, *__restrict__ iTf = p.iT;
   const double *__restrict__ rdz = p.rdz, *__restrict__ rhwt = p.rhw, *__restrict__ tabB = p.tabB;
   double *__restrict__ cp_scr = p.cp_scr;
 
-  const double dtau = p.dtau, b1 = p.b1, b2 = p.b2, g = p.g, gR = p.gR;
+  const double dtau = p.dtau, b1 = p.b1, b2 = p.b2, g = p.g, gR = p.gR, beta_d = p.beta_d;
   const double cU = dtau * gR * 0.5 * p.rdx, cV = dtau * gR * 0.5 * p.rdy;
   const double hx = 0.5 * p.rdx, hy = 0.5 * p.rdy;  // face theta = 0.5 (a + b), folded with 1/dx
   const double s = dtau * dtau * b2 * b2;
   const double sg2 = s * g * 0.5;
 
+  // S'' at one point (L581): 0 in RK stage 1, S^n - S^t at the first substep of a stage, else stored
+  auto pert = [&](int f, const double *P, size_t a) -> double {
+    if (ZERO) return 0.0;
+    if (FIRST) return p.Sn[f][a] - p.St[f][a];
+    return P[a];
+  };
+  // Theta''_d (L144) [R:G6]; Theta''_prev = Theta'' at the start of a stage
+  auto thd = [&](size_t a) -> double {
+    if (ZERO) return 0.0;
+    if (FIRST) return p.Sn[TH][a] - p.St[TH][a];
+    const double t = p.Pt[a];
+    return t + beta_d * (t - p.Ptp[a]);
+  };
   auto load_fwd = [&](int k, FwdIn &q) {
     const size_t kk = (size_t)k * plane;
     const size_t a = kk + oc, axm = kk + oxm, axp = kk + oxp, aym = kk + oym, ayp = kk + oyp;
-    q.d_c = thd_in[a]; q.d_xm = thd_in[axm]; q.d_xp = thd_in[axp]; q.d_ym = thd_in[aym]; q.d_yp = thd_in[ayp];
+    if (FIRST) {
+      q.T_c = q.d_c = thd(a);
+    } else {
+      q.T_c = p.Pt[a];
+      q.d_c = q.T_c + beta_d * (q.T_c - p.Ptp[a]);
+    }
+    q.d_xm = thd(axm); q.d_xp = thd(axp); q.d_ym = thd(aym); q.d_yp = thd(ayp);
     q.pi_c = pi[a]; q.pi_xm = pi[axm]; q.pi_xp = pi[axp]; q.pi_ym = pi[aym]; q.pi_yp = pi[ayp];
     q.th_xm = theta[axm]; q.th_xp = theta[axp]; q.th_ym = theta[aym]; q.th_yp = theta[ayp];
-    q.U_c = U_in[a]; q.U_xp = U_in[axp]; q.RU_c = RU[a]; q.RU_xp = RU[axp];
-    q.V_c = V_in[a]; q.V_yp = V_in[ayp]; q.RV_c = RV[a]; q.RV_yp = RV[ayp];
+    q.U_c = pert(UU, p.Pu, a); q.U_xp = pert(UU, p.Pu, axp); q.RU_c = RU[a]; q.RU_xp = RU[axp];
+    q.V_c = pert(VV, p.Pv, a); q.V_yp = pert(VV, p.Pv, ayp); q.RV_c = RV[a]; q.RV_yp = RV[ayp];
     const bool top = k + 1 >= nz;
     q.th_t = top ? 0.0 : theta[a + plane];
-    q.om_t = top ? 0.0 : Wf[a + plane];
-    q.RW = RW[a]; q.Tpp = Thf[a]; q.rpp = rhof[a]; q.RTh = RTh[a]; q.Rrho = Rrho[a]; q.iT = iTf[a];
+    q.om_t = top ? 0.0 : pert(WW, p.Pw, a + plane);
+    q.RW = RW[a]; q.rpp = pert(RHO, p.Pr, a); q.RTh = RTh[a]; q.Rrho = Rrho[a]; q.iT = iTf[a];
+    q.sU = LAST ? p.St[UU][a] : 0.0;
+    q.sV = LAST ? p.St[VV][a] : 0.0;
   };
 
   // ---------------- forward sweep: k = 0 .. nz-1 ----------------
@@ -99,15 +104,10 @@ __global__ void __launch_bounds__(32 * ROWS, MINB) k_acoustic_flat(const AcFlat 
   double That_m = 0.0, rhat_m = 0.0, cp_m = 0.0, dp_m = 0.0;
   double om_b = 0.0;                 // Omega''(k) = W''(k) at the end of the previous substep (0 on the lid)
   double th_c = theta[oc];           // theta^t(k)
-  FwdIn cur, nxt;
-  if (PF) load_fwd(0, cur);
+  FwdIn cur;
 #pragma unroll 1
   for (int k = 0; k < nz; k++) {
-    if (PF) {
-      if (k + 1 < nz) load_fwd(k + 1, nxt);  // software pipeline: next level's loads fly during this level's math
-    } else {
-      load_fwd(k, cur);
-    }
+    load_fwd(k, cur);
     const size_t a = (size_t)k * plane + oc;
     const bool top = k + 1 >= nz;
     // explicit horizontal momenta (L585 rows 1-2) at the four faces of the column
@@ -122,7 +122,7 @@ __global__ void __launch_bounds__(32 * ROWS, MINB) k_acoustic_flat(const AcFlat 
     const double DhT = (Up * (th_c + cur.th_xp) - Um * (cur.th_xm + th_c)) * hx +
                        (Vp * (th_c + cur.th_yp) - Vm * (cur.th_ym + th_c)) * hy;
     const double Dh = (Up - Um) * p.rdx + (Vp - Vm) * p.rdy;
-    const double Tpp = cur.Tpp, rpp = cur.rpp;
+    const double Tpp = cur.T_c, rpp = cur.rpp;
     const double Ttil = Tpp + dtau * (cur.RTh - DhT - b1 * (thf_t * om_t - thf_b * om_b) * rhc);
     const double rtil = rpp + dtau * (cur.Rrho - Dh - b1 * (om_t - om_b) * rhc);
     const double That = b2 * Ttil + b1 * Tpp, rhat = b2 * rtil + b1 * rpp;
@@ -145,14 +145,14 @@ __global__ void __launch_bounds__(32 * ROWS, MINB) k_acoustic_flat(const AcFlat 
       const double minv = 1.0 / (Dc - Ac * cp_m);
       cp_m = Cc * minv;
       dp_m = (rhs - Ac * dp_m) * minv;
-      if (CP_SMEM) s_cp[k * nthr + tid] = cp_m;
-      else cp_scr[a] = cp_m;
-      Wf[a] = dp_m;  // parked until the backward sweep
+      cp_scr[a] = cp_m;
+      p.kW[a] = dp_m;  // parked until the backward sweep
     }
-    U_out[a] = Um;
-    V_out[a] = Vm;
-    thd_out[a] = Ttil;  // parked
-    rhof[a] = rtil;     // parked
+    p.oU[a] = LAST ? cur.sU + Um : Um;
+    p.oV[a] = LAST ? cur.sV + Vm : Vm;
+    if (FIRST && !LAST && !ZERO) p.oTp[a] = cur.d_c;  // Theta''_prev of the next substep
+    p.kT[a] = Ttil;  // parked
+    p.kR[a] = rtil;  // parked
     pi_m = pi_c;
     th_c = cur.th_t;
     thf_bm = thf_b;
@@ -163,27 +163,32 @@ __global__ void __launch_bounds__(32 * ROWS, MINB) k_acoustic_flat(const AcFlat 
     That_m = That;
     rhat_m = rhat;
     om_b = om_t;
-    if (PF) cur = nxt;
   }
   // ---------------- backward sweep: k = nz-1 .. 0 ----------------
   struct BwdIn {
-    double dp, cp, Ttil, rtil, Told, thm;
+    double dp, cp, Ttil, rtil, thm, sW, sT, sR;
   };
   auto load_bwd = [&](int k, BwdIn &q) {
     const size_t a = (size_t)k * plane + oc;
     if (k >= 1) {
-      q.dp = Wf[a];
-      q.cp = CP_SMEM ? s_cp[k * nthr + tid] : cp_scr[a];
+      q.dp = p.kW[a];
+      q.cp = cp_scr[a];
       q.thm = theta[a - plane];
     } else {
       q.dp = 0.0; q.cp = 0.0; q.thm = 0.0;
     }
-    q.Ttil = thd_out[a]; q.rtil = rhof[a]; q.Told = Thf[a];
+    q.Ttil = p.kT[a]; q.rtil = p.kR[a];
+    if (LAST) {
+      q.sW = p.St[WW][a]; q.sT = p.St[TH][a]; q.sR = p.St[RHO][a];
+    } else {
+      q.sW = q.sT = q.sR = 0.0;
+    }
   };
   double On_t = 0.0;  // Omega''new(k+1); lid: 0
   double thc = theta[(size_t)(nz - 1) * plane + oc];
   double thft = 0.0;  // theta^t at face k+1
   const double cb = dtau * b2;
+  if (LAST) p.oW[(size_t)nz * plane + oc] = 0.0;  // flat lid: W = 0 at k = nz
   BwdIn ring[BD];  // modulo-scheduled ring: ring[n] holds level kb - n
 #pragma unroll
   for (int n = 0; n < BD; n++)
@@ -205,10 +210,15 @@ __global__ void __launch_bounds__(32 * ROWS, MINB) k_acoustic_flat(const AcFlat 
         const double rhc = rdz[k];
         const double Tnew = bc.Ttil - cb * (thft * On_t - thfb * On_b) * rhc;
         const double rnew = bc.rtil - cb * (On_t - On_b) * rhc;
-        if (k >= 1) Wf[a] = On_b;  // W'' = Omega'' on a flat grid
-        Thf[a] = Tnew;
-        rhof[a] = rnew;
-        thd_out[a] = Tnew + p.beta_d * (Tnew - bc.Told);  // divergence damping for the next substep (L144) [R:G6]
+        if (LAST) {
+          p.oW[a] = k >= 1 ? bc.sW + On_b : 0.0;  // L593; flat lid: W = 0 at k = 0
+          p.oT[a] = bc.sT + Tnew;
+          p.oR[a] = bc.sR + rnew;
+        } else {
+          if (k >= 1) p.oW[a] = On_b;  // W'' = Omega'' on a flat grid
+          p.oT[a] = Tnew;
+          p.oR[a] = rnew;
+        }
         On_t = On_b;
         thft = thfb;
         thc = bc.thm;
@@ -217,52 +227,15 @@ __global__ void __launch_bounds__(32 * ROWS, MINB) k_acoustic_flat(const AcFlat 
   }
 }
 
-void launch_acoustic_flat(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st) {
-  (void)St;
-  FusedState *z = c->fz;
-  AcFlat p;
-  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
-  p.dtau = dtau; p.rdx = 1.0 / c->v.dx; p.rdy = 1.0 / c->v.dy;
-  p.b1 = 0.5 * (1.0 - c->v.beta_s); p.b2 = 0.5 * (1.0 + c->v.beta_s);  // L589
-  p.beta_d = c->v.beta_d; p.g = c->v.g; p.gR = c->v.gam * c->v.Rd;
-  p.W = c->P.f[WW]; p.rho = c->P.f[RHO]; p.Th = c->P.f[TH];
-  p.RU = c->R.f[UU]; p.RV = c->R.f[VV]; p.RW = c->R.f[WW]; p.Rrho = c->R.f[RHO]; p.RTh = c->R.f[TH];
-  p.theta = c->theta_t; p.pi = c->pi_t; p.iT = z->iT;
-  p.rdz = z->tab.rdz; p.rhw = z->tab.rhw; p.tabB = z->tab.tabB;
-  p.cp_scr = z->cp_scr;
+void launch_acoustic_flat_one(const AcArgs &p, int mode, cudaStream_t st) {
   constexpr int ROWS = 4;
-  dim3 block(32, ROWS), grid((c->nx + 31) / 32, (c->ny + ROWS - 1) / ROWS);
-  size_t smem = (size_t)c->nz * 32 * ROWS * sizeof(double);
-  // variant bits (developer knob): 1 = forward prefetch, 2 = c' scratch in shared memory, 4 = allow 255 registers
-  const int var = z->variant;
-  bool cp_smem = smem <= 200 * 1024 && (var & 2);
-  auto kern = k_acoustic_flat<ROWS, false, 0, 4>;
-  switch (var & 7) {
-    case 1: kern = k_acoustic_flat<ROWS, false, 1, 4>; break;
-    case 2: kern = k_acoustic_flat<ROWS, true, 0, 4>; break;
-    case 3: kern = k_acoustic_flat<ROWS, true, 1, 4>; break;
-    case 4: kern = k_acoustic_flat<ROWS, false, 0, 1>; break;
-    case 5: kern = k_acoustic_flat<ROWS, false, 1, 1>; break;
-    case 6: kern = k_acoustic_flat<ROWS, true, 0, 1>; break;
-    case 7: kern = k_acoustic_flat<ROWS, true, 1, 1>; break;
-    default: break;
-  }
-  if (!cp_smem) smem = 0;
-  else cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  int cur = 0;
-  for (int sidx = 0; sidx < n; sidx++) {
-    Timed t(c, T_ACOUSTIC_FUSED, st);
-    p.thd_in = z->Thd[cur]; p.thd_out = z->Thd[cur ^ 1];
-    p.U_in = c->P.f[UU]; p.V_in = c->P.f[VV]; p.U_out = z->U2; p.V_out = z->V2;
-    kern<<<grid, block, smem, st>>>(p);
-    c->launches++;
-    // the new U'', V'' are the current ones: swap buffers
-    double *t1 = c->P.f[UU]; c->P.f[UU] = z->U2; z->U2 = t1;
-    double *t2 = c->P.f[VV]; c->P.f[VV] = z->V2; z->V2 = t2;
-    cur ^= 1;
-  }
-  if (cur) {  // keep Thd[0] the live buffer
-    double *t = z->Thd[0]; z->Thd[0] = z->Thd[1]; z->Thd[1] = t;
+  dim3 block(32, ROWS), grid((p.nx + 31) / 32, (p.ny + ROWS - 1) / ROWS);
+  switch (mode) {
+    case 0: k_acoustic_flat<ROWS, 0><<<grid, block, 0, st>>>(p); break;
+    case MODE_FIRST: k_acoustic_flat<ROWS, MODE_FIRST><<<grid, block, 0, st>>>(p); break;
+    case MODE_LAST: k_acoustic_flat<ROWS, MODE_LAST><<<grid, block, 0, st>>>(p); break;
+    case MODE_FIRST | MODE_LAST: k_acoustic_flat<ROWS, MODE_FIRST | MODE_LAST><<<grid, block, 0, st>>>(p); break;
+    default: k_acoustic_flat<ROWS, MODE_FIRST | MODE_LAST | MODE_ZERO><<<grid, block, 0, st>>>(p); break;
   }
 }
 
