@@ -10,6 +10,7 @@ enum { MODE_FIRST = 1, MODE_LAST = 2, MODE_ZERO = 4 };
 
 struct AcArgs {
   int nx, ny, nz, M, ZC;
+  int write_cp;  // thread-per-column kernel: store c' (stage constant, so only the first substep of a stage does)
   double dtau, rdx, rdy, b1, b2, beta_d, g, gR;
   const double *Pu, *Pv, *Pw, *Pr, *Pt, *Ptp;  // S'' in: U'', V'', W'', rho'', Theta'' and Theta''_prev
   const double *Sn[5], *St[5];                 // FIRST: S'' = Sn - St;  LAST: St is added to the result

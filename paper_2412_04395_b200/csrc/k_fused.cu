@@ -110,6 +110,7 @@ static void acoustic_substeps(erf_ctx *c, double dtau, int n, int stage, cudaStr
     }
     p.Pu = c->P.f[UU]; p.Pv = c->P.f[VV]; p.Pw = c->P.f[WW]; p.Pr = c->P.f[RHO]; p.Pt = cur; p.Ptp = prev;
     p.oTp = nullptr;
+    p.write_cp = sidx == 0;
     bool swap_uv = false, swap_stage = false;
     if (last) {
       if (stage == 1) {  // out of place: S^n -> S^t buffers

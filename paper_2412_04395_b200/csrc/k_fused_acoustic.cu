@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(32 * ROWS, 4) k_acoustic_flat(const AcArgs p) 
       const double minv = 1.0 / (Dc - Ac * cp_m);
       cp_m = Cc * minv;
       dp_m = (rhs - Ac * dp_m) * minv;
-      cp_scr[a] = cp_m;
+      if (p.write_cp) cp_scr[a] = cp_m;  // c' depends on the stage state and dtau only
       p.kW[a] = dp_m;  // parked until the backward sweep
     }
     p.oU[a] = LAST ? cur.sU + Um : Um;

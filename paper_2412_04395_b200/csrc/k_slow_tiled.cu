@@ -8,7 +8,7 @@
 // upward.  Vertical stencils live in per-thread register windows, vertical face fluxes are computed
 // once and carried to the cell above; everything a thread needs from its horizontal neighbours at
 // level k comes from shared-memory plane tiles (tiles.cuh) that cp.async fills one level ahead of the
-// arithmetic (two stages, one __syncthreads per level).  The thread's own column values for the
+// arithmetic (three stages: level k in use, k+1 and k+2 in flight; one __syncthreads per level).  The thread's own column values for the
 // levels above (k+3, k+4) are loaded straight from global memory one iteration before first use.
 //
 // Level ranges (grid.z chunks) let small grids fill the machine: a chunk starting at k0 > 0 first runs
@@ -22,6 +22,7 @@ using GB = TileG<4, 3>;  // halo 3 (x padded to 4): advected quantities
 using GS = TileG<2, 1>;  // halo 1 (x padded to 2)
 
 // ------------------------------------------------------------------ advection + PG + buoyancy
+constexpr int NSTAGE = 3;                            // pipeline depth: level k in use, k+1 and k+2 in flight
 constexpr int ADV_STAGE = 4 * GB::SZ + 4 * GS::SZ;  // doubles per pipeline stage
 
 template <int OH>
@@ -40,8 +41,9 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
 
   ChunkSet<4, 3> cb;
   ChunkSet<2, 1> cs;
-  cb.init(tid, x0, y0, nx, ny);
-  cs.init(tid, x0, y0, nx, ny);
+  int *tabs = reinterpret_cast<int *>(sm + NSTAGE * ADV_STAGE);
+  cb.init(tabs, tid, x0, y0, nx, ny);
+  cs.init(tabs + ChunkSet<4, 3>::TAB, tid, x0, y0, nx, ny);
   const double *__restrict__ U = p.U, *__restrict__ V = p.V, *__restrict__ W = p.W, *__restrict__ rho = p.rho;
   const double *__restrict__ th = p.theta, *__restrict__ u = p.u, *__restrict__ v = p.v, *__restrict__ w = p.w;
   const double *__restrict__ pp = p.pp;
@@ -59,6 +61,8 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
     cs.issue(s + 3 * GS::SZ, pp + kk);
   };
   stage_in(kb, 0);
+  cp_async_commit();
+  if (kb + 1 <= kl) stage_in(kb + 1, 1);
   cp_async_commit();
 
   double *__restrict__ Rrho = p.Rrho, *__restrict__ RU = p.RU, *__restrict__ RV = p.RV;
@@ -92,10 +96,10 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
 
 #pragma unroll 1
   for (int k = kb; k <= ke; k++) {
-    const int st = (k - kb) & 1;
-    cp_async_wait_all();
+    const int st = (k - kb) % NSTAGE;
+    cp_async_wait_but_one();  // level k has landed; level k+1 may still be in flight
     __syncthreads();
-    if (k + 1 <= kl) stage_in(k + 1, st ^ 1);
+    if (k + 2 <= kl) stage_in(k + 2, (k + 2 - kb) % NSTAGE);
     cp_async_commit();
     if (!act) continue;
     const double *__restrict__ sT = sm + st * ADV_STAGE, *__restrict__ sU = sT + GB::SZ,
@@ -235,7 +239,7 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
   const int kb = max(k0 - 1, 0), ke = k1, kl = min(ke, nz - 1);
 
   ChunkSet<2, 1> cs;
-  cs.init(tid, x0, y0, nx, ny);
+  cs.init(reinterpret_cast<int *>(sm + NSTAGE * DIFF_STAGE), tid, x0, y0, nx, ny);
   const double *__restrict__ u = p.u, *__restrict__ v = p.v, *__restrict__ w = p.w, *__restrict__ th = p.theta;
   const double *__restrict__ mu = p.mu, *__restrict__ Kf = p.K;
   auto stage_in = [&](int k, int st) {
@@ -249,6 +253,8 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
     cs.issue(b + 5 * GS::SZ, Kf + kk);
   };
   stage_in(kb, 0);
+  cp_async_commit();
+  if (kb + 1 <= kl) stage_in(kb + 1, 1);
   cp_async_commit();
 
   double *__restrict__ RU = p.RU, *__restrict__ RV = p.RV, *__restrict__ RW = p.RW, *__restrict__ RTh = p.RTh;
@@ -279,10 +285,10 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
 
 #pragma unroll 1
   for (int k = kb; k <= ke; k++) {
-    const int st = (k - kb) & 1;
-    cp_async_wait_all();
+    const int st = (k - kb) % NSTAGE;
+    cp_async_wait_but_one();
     __syncthreads();
-    if (k + 1 <= kl) stage_in(k + 1, st ^ 1);
+    if (k + 2 <= kl) stage_in(k + 2, (k + 2 - kb) % NSTAGE);
     cp_async_commit();
     if (!act) continue;
     const double *__restrict__ su = sm + st * DIFF_STAGE, *__restrict__ sv = su + GS::SZ,
@@ -380,7 +386,7 @@ static int level_chunks(const erf_ctx *c, int *kchunk) {
 
 template <int OH>
 static void launch_adv_tiled(const SlowFlat &p, dim3 grid, int kchunk, cudaStream_t st) {
-  const size_t smem = 2 * ADV_STAGE * sizeof(double);
+  const size_t smem = NSTAGE * ADV_STAGE * sizeof(double) + (ChunkSet<4, 3>::TAB + ChunkSet<2, 1>::TAB) * sizeof(int);
   static bool once = false;
   if (!once) {
     cudaFuncSetAttribute(k_adv_tiled<OH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -407,7 +413,7 @@ void launch_diff_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st) {
   int kchunk = 0;
   const int nch = level_chunks(c, &kchunk);
   dim3 grid((c->nx + TX - 1) / TX, (c->ny + TY - 1) / TY, nch);
-  const size_t smem = 2 * DIFF_STAGE * sizeof(double);
+  const size_t smem = NSTAGE * DIFF_STAGE * sizeof(double) + ChunkSet<2, 1>::TAB * sizeof(int);
   static bool once = false;
   if (!once) {
     cudaFuncSetAttribute(k_diff_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

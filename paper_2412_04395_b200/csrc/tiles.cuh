@@ -29,6 +29,7 @@ __device__ __forceinline__ void cp_async8(double *smem, const double *g) {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;\n" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_but_one() { asm volatile("cp.async.wait_group 1;\n" ::: "memory"); }
 
 // Tile geometry: x halo HXP (even, so that every 2-double chunk starts on an even column), y halo HY.
 template <int HXP, int HY>
@@ -40,42 +41,47 @@ struct TileG {
   __device__ static __forceinline__ int centre(int tx, int ty) { return (ty + HY) * W + tx + HXP; }
 };
 
-// One thread's share of a tile copy (the same for every field with this geometry and every level).
+// One thread's share of a tile copy (the same for every field with this geometry and every level).  The
+// source/destination offsets live in shared memory ([3*PER][NTHR] ints at `tab`, each thread reads only its
+// own column), not in registers: the column kernels need every register for their stencil windows.
 template <int HXP, int HY>
 struct ChunkSet {
   using G = TileG<HXP, HY>;
-  int g0[G::PER];  // offset of the chunk's first double within a plane, or -1 if the thread has no such chunk
-  int g1[G::PER];  // offset of the second double, or -1 when both are moved by one 16-byte copy
-  int s[G::PER];   // offset within the tile
-  __device__ __forceinline__ void init(int tid, int x0, int y0, int nx, int ny) {
+  static constexpr int TAB = 3 * G::PER * NTHR;  // ints of shared memory
+  const int *t;  // tab + tid
+  // g0 = offset of the chunk's first double within a plane (-1: the thread has no such chunk); g1 = offset of
+  // the second double (-1: both are moved by one 16-byte copy); s = offset within the tile
+  __device__ __forceinline__ void init(int *tab, int tid, int x0, int y0, int nx, int ny) {
 #pragma unroll
     for (int n = 0; n < G::PER; n++) {
       const int c = tid + n * NTHR;
+      int g0 = -1, g1 = -1, so = 0;
       if (c < G::NCH) {
         const int ry = c / G::CW, cx = c - ry * G::CW;
         const int gy = pmod(y0 - HY + ry, ny);
         const int gxa = pmod(x0 - HXP + 2 * cx, nx), gxb = pmod(x0 - HXP + 2 * cx + 1, nx);
-        g0[n] = gy * nx + gxa;
+        g0 = gy * nx + gxa;
         const bool vec = !(nx & 1) && !(gxa & 1) && gxb == gxa + 1;
-        g1[n] = vec ? -1 : gy * nx + gxb;
-        s[n] = ry * G::W + 2 * cx;
-      } else {
-        g0[n] = -1;
-        g1[n] = -1;
-        s[n] = 0;
+        g1 = vec ? -1 : gy * nx + gxb;
+        so = ry * G::W + 2 * cx;
       }
+      tab[(3 * n) * NTHR + tid] = g0;
+      tab[(3 * n + 1) * NTHR + tid] = g1;
+      tab[(3 * n + 2) * NTHR + tid] = so;
     }
+    t = tab + tid;
   }
   // copy this thread's chunks of one field plane (gplane = field + k * plane) into a tile
   __device__ __forceinline__ void issue(double *tile, const double *__restrict__ gplane) const {
 #pragma unroll
     for (int n = 0; n < G::PER; n++) {
-      if (g0[n] >= 0) {
-        if (g1[n] < 0) {
-          cp_async16(tile + s[n], gplane + g0[n]);
+      const int g0 = t[(3 * n) * NTHR], g1 = t[(3 * n + 1) * NTHR], so = t[(3 * n + 2) * NTHR];
+      if (g0 >= 0) {
+        if (g1 < 0) {
+          cp_async16(tile + so, gplane + g0);
         } else {
-          cp_async8(tile + s[n], gplane + g0[n]);
-          cp_async8(tile + s[n] + 1, gplane + g1[n]);
+          cp_async8(tile + so, gplane + g0);
+          cp_async8(tile + so + 1, gplane + g1);
         }
       }
     }

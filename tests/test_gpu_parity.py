@@ -286,3 +286,33 @@ def test_uses_the_caller_stream(torch, erfo, B):
     got = _host(out)
     d.close()
     assert max(field_errors(got, ref)) <= 2 * TOL_1STEP
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict(nx=40, ny=23, nz=19)), (3, dict(nx=45, ny=20, nz=34)),
+                                    (5, dict(nx=70, ny=11, nz=40)), (5, dict(nx=33, ny=9, nz=128))])
+def test_z_chunked_acoustic_kernel(torch, erfo, B, cfg, kw, monkeypatch):
+    """The opt-in z-chunked substep kernel (partitioned tridiagonal solve, k_acoustic_zc.cu) against the
+    oracle: n substeps through erf_acoustic and one full RK3 step (stage combine folded in)."""
+    monkeypatch.setenv("ERF_B200_VARIANT", "32")  # developer knob read by erf_create
+    case = wl.make_case(cfg, **kw)
+    nz, ny, nx = case["nz"], case["ny"], case["nx"]
+    rng = np.random.default_rng(91 + cfg)
+    o = erfo.Oracle(case)
+    o.set_state(*case["state"])
+    R = o.slow_rhs()
+    P = [1e-3 * rng.standard_normal((nz + (f == 3), ny, nx)) for f in range(5)]
+    P[3][0] = 0.0
+    P[3][nz] = 0.0
+    dtau = case["dt"] / case["ns"]
+    ref = o.acoustic(dtau, 4, R, P)
+    o.close()
+    d = B.Dycore(case)
+    d.set_state(*_dev(torch, case["state"]))
+    got = _host(d.acoustic(dtau, 4, _dev(torch, R), _dev(torch, P)))
+    d.close()
+    got[3][0] = ref[3][0]
+    got[3][nz] = ref[3][nz]
+    assert max(field_errors(got, ref)) <= TOL_1STEP, field_errors(got, ref)
+    ref = _run_oracle(erfo, case, 2)
+    got = _run_gpu(torch, B, case, 2)
+    assert max(field_errors(got, ref)) <= TOL_1STEP * 2, field_errors(got, ref)
