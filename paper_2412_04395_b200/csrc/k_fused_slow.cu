@@ -392,11 +392,12 @@ void launch_slow_flat(erf_ctx *c, const F5 &S, cudaStream_t st) {
     c->launches++;
   }
   if (c->p.diffusion != 0) {
-    k_visc_flat<<<(unsigned)((plane * c->nz + 255) / 256), 256, 0, st>>>(p);
-    c->launches++;
     if (tiled) {
+      launch_visc_tiled(c, p, st);
       launch_diff_tiled(c, p, st);
     } else {
+      k_visc_flat<<<(unsigned)((plane * c->nz + 255) / 256), 256, 0, st>>>(p);
+      c->launches++;
       k_diff_flat<<<grid, block, 0, st>>>(p);
       c->launches++;
     }

@@ -23,10 +23,18 @@ using GS = TileG<2, 1>;  // halo 1 (x padded to 2)
 
 // ------------------------------------------------------------------ advection + PG + buoyancy
 constexpr int NSTAGE = 3;                            // pipeline depth: level k in use, k+1 and k+2 in flight
-constexpr int ADV_STAGE = 4 * GB::SZ + 4 * GS::SZ;  // doubles per pipeline stage
+// doubles per pipeline stage: one halo-3 tile per advected field of the launch, then the U, V, W, p' tiles
+__host__ __device__ constexpr int adv_stage(int fm) { return ((fm & 1) + ((fm >> 1) & 1) + ((fm >> 2) & 1) + ((fm >> 3) & 1)) * GB::SZ + 4 * GS::SZ; }
 
-template <int OH>
-__global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const int kchunk) {
+// FM = field mask: which tendencies this launch computes.  One launch with all four bits computes everything;
+// splitting by field trades re-reading the mass-flux tiles for much lower register pressure per launch.
+enum { F_T = 1, F_U = 2, F_V = 4, F_W = 8, F_ALL = 15 };  // F_T: rho and rho*theta; F_W: rho*w with PG_z + buoyancy
+
+template <int OH, int FM>
+__global__ void __launch_bounds__(NTHR, FM == F_ALL ? 2 : 3) k_adv_tiled(const SlowFlat p, const int kchunk) {
+  constexpr bool DO_T = (FM & F_T) != 0, DO_U = (FM & F_U) != 0, DO_V = (FM & F_V) != 0, DO_W = (FM & F_W) != 0;
+  constexpr int ADV_STAGE = adv_stage(FM);
+  constexpr int OFF_U = DO_T * GB::SZ, OFF_V = OFF_U + DO_U * GB::SZ, OFF_W = OFF_V + DO_V * GB::SZ, OFF_S = OFF_W + DO_W * GB::SZ;
   extern __shared__ __align__(16) double sm[];
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
   const int nx = p.nx, ny = p.ny, nz = p.nz, ov = p.ov;
@@ -50,15 +58,15 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
   auto stage_in = [&](int k, int st) {
     double *b = sm + st * ADV_STAGE;
     const size_t kk = (size_t)k * plane;
-    cb.issue(b, th + kk);
-    cb.issue(b + GB::SZ, u + kk);
-    cb.issue(b + 2 * GB::SZ, v + kk);
-    cb.issue(b + 3 * GB::SZ, w + kk);
-    double *s = b + 4 * GB::SZ;
+    if (DO_T) cb.issue(b, th + kk);
+    if (DO_U) cb.issue(b + OFF_U, u + kk);
+    if (DO_V) cb.issue(b + OFF_V, v + kk);
+    if (DO_W) cb.issue(b + OFF_W, w + kk);
+    double *s = b + OFF_S;
     cs.issue(s, U + kk);
     cs.issue(s + GS::SZ, V + kk);
-    cs.issue(s + 2 * GS::SZ, W + kk);
-    cs.issue(s + 3 * GS::SZ, pp + kk);
+    if (DO_U || DO_V) cs.issue(s + 2 * GS::SZ, W + kk);
+    if (DO_U || DO_V || DO_W) cs.issue(s + 3 * GS::SZ, pp + kk);
   };
   stage_in(kb, 0);
   cp_async_commit();
@@ -79,10 +87,10 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
     const int kc = kb + n - 3, kf = kb + n - 2;
     const bool okc = act && kc >= 0 && kc < nz, okf = act && kf >= 0 && kf <= nz;
     const size_t ac = (size_t)(okc ? kc : 0) * plane + oc, af = (size_t)(okf ? kf : 0) * plane + oc;
-    wt[n] = okc ? th[ac] : 0.0;
-    wu[n] = okc ? u[ac] : 0.0;
-    wv[n] = okc ? v[ac] : 0.0;
-    ww[n] = okf ? w[af] : 0.0;
+    wt[n] = (DO_T && okc) ? th[ac] : 0.0;
+    wu[n] = (DO_U && okc) ? u[ac] : 0.0;
+    wv[n] = (DO_V && okc) ? v[ac] : 0.0;
+    ww[n] = (DO_W && okf) ? w[af] : 0.0;
   }
   double fT_b = 0.0, fU_b = 0.0, fV_b = 0.0, om_b = 0.0;  // face fluxes at the bottom of the previous cell
   double HT = 0.0, HU = 0.0, HV = 0.0, Hr = 0.0;          // horizontal parts of the previous cell
@@ -92,7 +100,7 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
   double om_c = (act && kb >= 1) ? W[(size_t)kb * plane + oc] : 0.0;  // Omega at face k (lid: 0)
   // prefetched one iteration ahead: Omega at face k+1, rho at cell k
   double om_n = (act && kb + 1 <= nz - 1) ? W[(size_t)(kb + 1) * plane + oc] : 0.0;
-  double rho_n = act ? rho[(size_t)kb * plane + oc] : 0.0;
+  double rho_n = (DO_W && act) ? rho[(size_t)kb * plane + oc] : 0.0;
 
 #pragma unroll 1
   for (int k = kb; k <= ke; k++) {
@@ -102,9 +110,9 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
     if (k + 2 <= kl) stage_in(k + 2, (k + 2 - kb) % NSTAGE);
     cp_async_commit();
     if (!act) continue;
-    const double *__restrict__ sT = sm + st * ADV_STAGE, *__restrict__ sU = sT + GB::SZ,
-                               *__restrict__ sV = sT + 2 * GB::SZ, *__restrict__ sW = sT + 3 * GB::SZ;
-    const double *__restrict__ mU = sT + 4 * GB::SZ, *__restrict__ mV = mU + GS::SZ,
+    const double *__restrict__ sT = sm + st * ADV_STAGE, *__restrict__ sU = sT + OFF_U,
+                               *__restrict__ sV = sT + OFF_V, *__restrict__ sW = sT + OFF_W;
+    const double *__restrict__ mU = sT + OFF_S, *__restrict__ mV = mU + GS::SZ,
                                *__restrict__ mW = mU + 2 * GS::SZ, *__restrict__ mP = mU + 3 * GS::SZ;
     const size_t kk = (size_t)k * plane;
     // own-column values for the next iteration (window tops, Omega at face k+2, rho at cell k+1)
@@ -113,34 +121,35 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
       const int kc = k + 3, kf = k + 4;
       if (kc < nz) {
         const size_t ac = (size_t)kc * plane + oc;
-        nt = th[ac];
-        nu_ = u[ac];
-        nv = v[ac];
+        if (DO_T) nt = th[ac];
+        if (DO_U) nu_ = u[ac];
+        if (DO_V) nv = v[ac];
       }
-      if (kf <= nz) nw = w[(size_t)kf * plane + oc];
+      if (DO_W && kf <= nz) nw = w[(size_t)kf * plane + oc];
       if (k + 2 <= nz - 1) om_nn = W[(size_t)(k + 2) * plane + oc];
-      if (k + 1 < nz) rho_nn = rho[(size_t)(k + 1) * plane + oc];
+      if (DO_W && k + 1 < nz) rho_nn = rho[(size_t)(k + 1) * plane + oc];
     }
     // ---- face k: vertical fluxes of theta, u, v (zero on the lids)
     double fT = 0.0, fU = 0.0, fV = 0.0;
     if (k >= 1 && k <= nz - 1) {
       const int ord = vorder(ov, min(k, nz - k));
-      const double om_xm = mW[cS - 1], om_ym = mW[cS - WS];
-      fT = flux_rt(ord, om_c, wt);
-      fU = flux_rt(ord, 0.5 * (om_xm + om_c), wu);
-      fV = flux_rt(ord, 0.5 * (om_ym + om_c), wv);
+      if (DO_T) fT = flux_rt(ord, om_c, wt);
+      if (DO_U) fU = flux_rt(ord, 0.5 * (mW[cS - 1] + om_c), wu);
+      if (DO_V) fV = flux_rt(ord, 0.5 * (mW[cS - WS] + om_c), wv);
     }
     // ---- finish cell k-1
     if (k - 1 >= k0) {
       const size_t am = kk - plane + oc;
       const double rdzm = p.rdz[k - 1];
-      Rrho[am] = -(Hr + (om_c - om_b) * rdzm);
-      RTh[am] = -(HT + (fT - fT_b) * rdzm);
-      RU[am] = -(HU + (fU - fU_b) * rdzm);
-      RV[am] = -(HV + (fV - fV_b) * rdzm);
+      if (DO_T) {
+        Rrho[am] = -(Hr + (om_c - om_b) * rdzm);
+        RTh[am] = -(HT + (fT - fT_b) * rdzm);
+      }
+      if (DO_U) RU[am] = -(HU + (fU - fU_b) * rdzm);
+      if (DO_V) RV[am] = -(HV + (fV - fV_b) * rdzm);
     }
     if (k == nz) {
-      RW[kk + oc] = 0.0;
+      if (DO_W) RW[kk + oc] = 0.0;
       continue;
     }
     if (k == ke) continue;  // the cell above belongs to the next chunk
@@ -150,8 +159,8 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
     const double U_ym = mU[cS - WS], U_pym = mU[cS - WS + 1];
     const double V_m1 = mV[cS - WS], V_c = mV[cS], V_p1 = mV[cS + WS];
     const double V_xm = mV[cS - 1], V_xmp = mV[cS + WS - 1];
-    Hr = (U_p1 - U_c) * rdx + (V_p1 - V_c) * rdy;
-    {
+    if (DO_T) Hr = (U_p1 - U_c) * rdx + (V_p1 - V_c) * rdy;
+    if (DO_T) {
       double q[7];
 #pragma unroll
       for (int n = 0; n < 7; n++) q[n] = sT[cB + n - 3];
@@ -160,8 +169,8 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
       for (int n = 0; n < 7; n++) q[n] = sT[cB + (n - 3) * WB];
       HT += (flux_c<OH>(V_p1, q[1], q[2], q[3], q[4], q[5], q[6]) - flux_c<OH>(V_c, q[0], q[1], q[2], q[3], q[4], q[5])) * rdy;
     }
-    const double pp_c = mP[cS];
-    {
+    const double pp_c = (DO_U || DO_V || DO_W) ? mP[cS] : 0.0;
+    if (DO_U) {
       double q[7];
 #pragma unroll
       for (int n = 0; n < 7; n++) q[n] = sU[cB + n - 3];
@@ -173,7 +182,7 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
              flux_c<OH>(0.5 * (V_xm + V_c), q[0], q[1], q[2], q[3], q[4], q[5])) * rdy;
       HU += (pp_c - mP[cS - 1]) * rdx;
     }
-    {
+    if (DO_V) {
       double q[7];
 #pragma unroll
       for (int n = 0; n < 7; n++) q[n] = sV[cB + n - 3];
@@ -187,6 +196,7 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
     }
     // ---- w equation at face k; vertical flux at centre k
     const double om_t = om_n;
+    if (DO_W) {
     const double Gz = flux_rt(vorder(ov, min(k + 1, nz - k)), 0.5 * (om_c + om_t), ww);
     const double dzk = p.dz[k];
     const double U_cd = dzk * U_c, U_pd = dzk * U_p1, V_cd = dzk * V_c, V_pd = dzk * V_p1;
@@ -210,13 +220,17 @@ __global__ void __launch_bounds__(NTHR, 2) k_adv_tiled(const SlowFlat p, const i
     Gz_m = Gz;
     U_cm = U_cd; U_pm = U_pd; V_cm = V_cd; V_pm = V_pd;
     pp_m = pp_c; rp_m = rp_c;
+    }
     om_c = om_t;
     om_n = om_nn;
     rho_n = rho_nn;
     // ---- shift the vertical windows: bring in cell k+3 and face k+4
 #pragma unroll
     for (int n = 0; n < 5; n++) {
-      wt[n] = wt[n + 1]; wu[n] = wu[n + 1]; wv[n] = wv[n + 1]; ww[n] = ww[n + 1];
+      if (DO_T) wt[n] = wt[n + 1];
+      if (DO_U) wu[n] = wu[n + 1];
+      if (DO_V) wv[n] = wv[n + 1];
+      if (DO_W) ww[n] = ww[n + 1];
     }
     wt[5] = nt; wu[5] = nu_; wv[5] = nv; ww[5] = nw;
   }
@@ -373,6 +387,103 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
   }
 }
 
+// ------------------------------------------------------------------ Smagorinsky viscosity
+// mu = rho nu + mu_t, K = rho alpha + mu_t / Pr_t; mu_t = rho (Cs Delta)^2 |S| (Eq. 9) [R:G9,G10].
+// Cell k needs u, v of levels k-1, k, k+1 and w of faces k, k+1 with a halo of one column: a ring of five
+// stages (stage L = u(L), v(L), w(face L+1)) holds levels k-1..k+1 while k+2 and k+3 are in flight.
+constexpr int VISC_NST = 5, VISC_STAGE = 3 * GS::SZ;
+
+__global__ void __launch_bounds__(NTHR, 4) k_visc_tiled(const SlowFlat p, const int kchunk) {
+  extern __shared__ __align__(16) double sm[];
+  const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
+  const int nx = p.nx, ny = p.ny, nz = p.nz;
+  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+  const int i = x0 + tx, j = y0 + ty;
+  const bool act = i < nx && j < ny;
+  const size_t plane = (size_t)nx * ny;
+  const int k0 = blockIdx.z * kchunk, k1 = min(nz, k0 + kchunk);  // this CTA's cells [k0, k1)
+  const int Lb = k0 - 1, Le = min(k1, nz - 1);                    // stages Lb .. Le are needed
+
+  ChunkSet<2, 1> cs;
+  cs.init(reinterpret_cast<int *>(sm + VISC_NST * VISC_STAGE), tid, x0, y0, nx, ny);
+  const double *__restrict__ u = p.u, *__restrict__ v = p.v, *__restrict__ w = p.w, *__restrict__ rho = p.rho;
+  auto slot = [&](int L) { return sm + ((L - Lb) % VISC_NST) * VISC_STAGE; };
+  auto stage_in = [&](int L) {
+    if (L > Le) return;
+    double *b = slot(L);
+    if (L >= 0) {
+      cs.issue(b, u + (size_t)L * plane);
+      cs.issue(b + GS::SZ, v + (size_t)L * plane);
+    }
+    cs.issue(b + 2 * GS::SZ, w + (size_t)(L + 1) * plane);  // face L+1 (L = -1: the lower lid)
+  };
+#pragma unroll
+  for (int n = 0; n < 4; n++) {
+    stage_in(Lb + n);
+    cp_async_commit();
+  }
+  constexpr int WS = GS::W;
+  const int c = GS::centre(tx, ty);
+  const size_t oc = act ? (size_t)j * nx + i : 0;
+  const double rdx = p.rdx, rdy = p.rdy;
+  double rho_n = act ? rho[(size_t)k0 * plane + oc] : 0.0;
+
+#pragma unroll 1
+  for (int k = k0; k < k1; k++) {
+    cp_async_wait_but_one();  // stages up to k+1 have landed; k+2 may still be in flight
+    __syncthreads();
+    stage_in(k + 3);          // into the slot of stage k-2, which every thread has finished reading
+    cp_async_commit();
+    if (!act) continue;
+    const double rc = rho_n;
+    if (k + 1 < k1) rho_n = rho[(size_t)(k + 1) * plane + oc];
+    double mu = rc * p.nu, K = rc * p.alpha;
+    if (p.diffusion == 2) {
+      const double *__restrict__ su = slot(k), *__restrict__ sv = su + GS::SZ, *__restrict__ swt = su + 2 * GS::SZ;
+      const double *__restrict__ sm1 = slot(k - 1), *__restrict__ sp1 = slot(k + 1);
+      const double *__restrict__ swb = sm1 + 2 * GS::SZ;  // w at face k
+      const double u_c = su[c], u_p = su[c + 1], v_c = sv[c], v_p = sv[c + WS];
+      const double S11 = (u_p - u_c) * rdx, S22 = (v_p - v_c) * rdy;
+      const double w_c = swb[c], w_t = swt[c];
+      const double S33 = (w_t - w_c) * p.rdz[k];
+      // S12 at the four xy-edges around the centre
+      const double u_jm = su[c - WS], u_jp = su[c + WS], u_pjm = su[c + 1 - WS], u_pjp = su[c + 1 + WS];
+      const double v_im = sv[c - 1], v_ip = sv[c + 1], v_imp = sv[c - 1 + WS], v_ipp = sv[c + 1 + WS];
+      const double e00 = 0.5 * ((u_c - u_jm) * rdy + (v_c - v_im) * rdx);
+      const double e10 = 0.5 * ((u_p - u_pjm) * rdy + (v_ip - v_c) * rdx);
+      const double e01 = 0.5 * ((u_jp - u_c) * rdy + (v_p - v_imp) * rdx);
+      const double e11 = 0.5 * ((u_pjp - u_p) * rdy + (v_ipp - v_p) * rdx);
+      const double s12 = 0.25 * (e00 + e10 + e01 + e11);
+      // S13 at (i,k), (i+1,k), (i,k+1), (i+1,k+1); S23 likewise; zero on the lids
+      double s13 = 0.0, s23 = 0.0;
+      if (k >= 1) {
+        const double rhw = p.rhw[k];
+        const double *__restrict__ um = sm1, *__restrict__ vm = sm1 + GS::SZ;
+        s13 += 0.5 * ((u_c - um[c]) * rhw + (w_c - swb[c - 1]) * rdx) +
+               0.5 * ((u_p - um[c + 1]) * rhw + (swb[c + 1] - w_c) * rdx);
+        s23 += 0.5 * ((v_c - vm[c]) * rhw + (w_c - swb[c - WS]) * rdy) +
+               0.5 * ((v_p - vm[c + WS]) * rhw + (swb[c + WS] - w_c) * rdy);
+      }
+      if (k + 1 <= nz - 1) {
+        const double rhw = p.rhw[k + 1];
+        const double *__restrict__ up = sp1, *__restrict__ vp = sp1 + GS::SZ;
+        s13 += 0.5 * ((up[c] - u_c) * rhw + (w_t - swt[c - 1]) * rdx) +
+               0.5 * ((up[c + 1] - u_p) * rhw + (swt[c + 1] - w_t) * rdx);
+        s23 += 0.5 * ((vp[c] - v_c) * rhw + (w_t - swt[c - WS]) * rdy) +
+               0.5 * ((vp[c + WS] - v_p) * rhw + (swt[c + WS] - w_t) * rdy);
+      }
+      s13 *= 0.25;
+      s23 *= 0.25;
+      const double ss = 2.0 * (S11 * S11 + S22 * S22 + S33 * S33) + 4.0 * (s12 * s12 + s13 * s13 + s23 * s23);
+      const double mut = rc * p.csd2[k] * sqrt(ss);
+      mu += mut;
+      K += mut * p.rPrt;
+    }
+    p.mu[(size_t)k * plane + oc] = mu;
+    p.K[(size_t)k * plane + oc] = K;
+  }
+}
+
 // number of level chunks so that a small grid still fills the machine (2 CTAs x 148 SMs, twice over)
 static int level_chunks(const erf_ctx *c, int *kchunk) {
   const int tiles = ((c->nx + TX - 1) / TX) * ((c->ny + TY - 1) / TY);
@@ -384,28 +495,72 @@ static int level_chunks(const erf_ctx *c, int *kchunk) {
   return (c->nz + *kchunk - 1) / *kchunk;
 }
 
-template <int OH>
-static void launch_adv_tiled(const SlowFlat &p, dim3 grid, int kchunk, cudaStream_t st) {
-  const size_t smem = NSTAGE * ADV_STAGE * sizeof(double) + (ChunkSet<4, 3>::TAB + ChunkSet<2, 1>::TAB) * sizeof(int);
+template <int OH, int FM>
+static void launch_adv_mask(const SlowFlat &p, dim3 grid, int kchunk, cudaStream_t st) {
+  const size_t smem = NSTAGE * adv_stage(FM) * sizeof(double) + (ChunkSet<4, 3>::TAB + ChunkSet<2, 1>::TAB) * sizeof(int);
   static bool once = false;
   if (!once) {
-    cudaFuncSetAttribute(k_adv_tiled<OH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(k_adv_tiled<OH, FM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     once = true;
   }
-  k_adv_tiled<OH><<<grid, dim3(TX, TY), smem, st>>>(p, kchunk);
+  k_adv_tiled<OH, FM><<<grid, dim3(TX, TY), smem, st>>>(p, kchunk);
+}
+
+// split: 0 = one launch for all five tendencies; 1 = (rho, Theta, W) + (U, V); 2 = (rho, Theta) + (U, V) + (W)
+// (the default: measured fastest on B200 -- 3 CTAs per SM without spills beat re-reading the U, V, W, p' tiles);
+// 3 = one launch per field
+template <int OH>
+static int launch_adv_tiled(const SlowFlat &p, dim3 grid, int kchunk, int split, cudaStream_t st) {
+  if (split == 1) {
+    launch_adv_mask<OH, F_T | F_W>(p, grid, kchunk, st);
+    launch_adv_mask<OH, F_U | F_V>(p, grid, kchunk, st);
+    return 2;
+  }
+  if (split == 2) {
+    launch_adv_mask<OH, F_T>(p, grid, kchunk, st);
+    launch_adv_mask<OH, F_U | F_V>(p, grid, kchunk, st);
+    launch_adv_mask<OH, F_W>(p, grid, kchunk, st);
+    return 3;
+  }
+  if (split == 3) {
+    launch_adv_mask<OH, F_T>(p, grid, kchunk, st);
+    launch_adv_mask<OH, F_U>(p, grid, kchunk, st);
+    launch_adv_mask<OH, F_V>(p, grid, kchunk, st);
+    launch_adv_mask<OH, F_W>(p, grid, kchunk, st);
+    return 4;
+  }
+  launch_adv_mask<OH, F_ALL>(p, grid, kchunk, st);
+  return 1;
 }
 
 void launch_adv_diff_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st) {
   int kchunk = 0;
   const int nch = level_chunks(c, &kchunk);
   dim3 grid((c->nx + TX - 1) / TX, (c->ny + TY - 1) / TY, nch);
+  const int knob = (c->fz->variant >> 6) & 3;  // developer knob: 0 default, 1 fused, 2 two-way, 3 four-way
+  const int split = knob == 0 ? 2 : (knob == 1 ? 0 : (knob == 2 ? 1 : 3));
+  int n = 1;
   switch (c->p.adv_order_h) {
-    case 2: launch_adv_tiled<2>(p, grid, kchunk, st); break;
-    case 3: launch_adv_tiled<3>(p, grid, kchunk, st); break;
-    case 4: launch_adv_tiled<4>(p, grid, kchunk, st); break;
-    case 5: launch_adv_tiled<5>(p, grid, kchunk, st); break;
-    default: launch_adv_tiled<6>(p, grid, kchunk, st); break;
+    case 2: n = launch_adv_tiled<2>(p, grid, kchunk, split, st); break;
+    case 3: n = launch_adv_tiled<3>(p, grid, kchunk, split, st); break;
+    case 4: n = launch_adv_tiled<4>(p, grid, kchunk, split, st); break;
+    case 5: n = launch_adv_tiled<5>(p, grid, kchunk, split, st); break;
+    default: n = launch_adv_tiled<6>(p, grid, kchunk, split, st); break;
   }
+  c->launches += n;
+}
+
+void launch_visc_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st) {
+  int kchunk = 0;
+  const int nch = level_chunks(c, &kchunk);
+  dim3 grid((c->nx + TX - 1) / TX, (c->ny + TY - 1) / TY, nch);
+  const size_t smem = VISC_NST * VISC_STAGE * sizeof(double) + ChunkSet<2, 1>::TAB * sizeof(int);
+  static bool once = false;
+  if (!once) {
+    cudaFuncSetAttribute(k_visc_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    once = true;
+  }
+  k_visc_tiled<<<grid, dim3(TX, TY), smem, st>>>(p, kchunk);
   c->launches++;
 }
 

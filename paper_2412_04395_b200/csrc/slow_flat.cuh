@@ -53,5 +53,6 @@ __device__ __forceinline__ int vorder(int req, int r) {
 // k_slow_tiled.cu
 void launch_adv_diff_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st);
 void launch_diff_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st);
+void launch_visc_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st);
 
 }  // namespace erfb
