@@ -48,6 +48,22 @@ def measured_peak_gbs():
         return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def measured_traffic(kernel_class, config):
+    """DRAM bytes per launch of a kernel class from the committed ncu capture of config 5
+    (profiles/r1_dram_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum); None for other workloads."""
+    if config != 5:
+        return None
+    import csv
+    try:
+        with open(os.path.join(ROOT, "profiles", "r1_dram_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if row["kernel_class"] == kernel_class:
+                    return float(row["bytes_per_launch"])
+    except Exception:
+        pass
+    return None
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons during the timed region (pynvml)."""
 
@@ -261,7 +277,7 @@ def run_ours(args):
             per_launch, units = alg_bytes["slow_rhs"], "one slow right-hand side"
         achieved = per_launch / (tot_ms / calls * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": name, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": measured_traffic(name, args.config), "peak_source": peak_src,
                 "launch_unit": units, "algorithmic_bytes_per_launch": per_launch,
                 "avg_launch_ms": tot_ms / calls,
                 "share_of_step": tot_ms / ms,
