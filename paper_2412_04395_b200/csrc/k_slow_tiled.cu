@@ -239,9 +239,14 @@ __global__ void __launch_bounds__(NTHR, FM == F_ALL ? 2 : 3) k_adv_tiled(const S
 // ------------------------------------------------------------------ diffusion
 // R_U,V,W -= div(tau), tau = -2 mu (S - 1/3 div u I) (Eq. 9); R_Theta -= div(-K grad theta) (Eq. 3);
 // free-slip lids: tau13 = tau23 = 0 and no scalar flux at k = 0, nz (Table C1 "Slip Wall").
-constexpr int DIFF_STAGE = 6 * GS::SZ;
+__host__ __device__ constexpr int diff_stage(int part) { return ((part & 1) ? 4 : 0) * GS::SZ + ((part & 2) ? 2 : 0) * GS::SZ; }
 
-__global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const int kchunk) {
+// PART bits: 1 = momentum (tiles u, v, w, mu), 2 = scalar (tiles theta, K); the two parts share no tile, so
+// splitting them costs no traffic and lets the scalar part run at high occupancy.
+template <int PART>
+__global__ void __launch_bounds__(NTHR, PART == 2 ? 4 : 2) k_diff_tiled(const SlowFlat p, const int kchunk) {
+  constexpr bool DO_M = (PART & 1) != 0, DO_S = (PART & 2) != 0;
+  constexpr int DIFF_STAGE = diff_stage(PART), OFF_TH = DO_M ? 4 * GS::SZ : 0, OFF_K = OFF_TH + GS::SZ;
   extern __shared__ __align__(16) double sm[];
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
   const int nx = p.nx, ny = p.ny, nz = p.nz;
@@ -259,12 +264,16 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
   auto stage_in = [&](int k, int st) {
     double *b = sm + st * DIFF_STAGE;
     const size_t kk = (size_t)k * plane;
-    cs.issue(b, u + kk);
-    cs.issue(b + GS::SZ, v + kk);
-    cs.issue(b + 2 * GS::SZ, w + kk + plane);  // w at face k+1
-    cs.issue(b + 3 * GS::SZ, th + kk);
-    cs.issue(b + 4 * GS::SZ, mu + kk);
-    cs.issue(b + 5 * GS::SZ, Kf + kk);
+    if (DO_M) {
+      cs.issue(b, u + kk);
+      cs.issue(b + GS::SZ, v + kk);
+      cs.issue(b + 2 * GS::SZ, w + kk + plane);  // w at face k+1
+      cs.issue(b + 3 * GS::SZ, mu + kk);
+    }
+    if (DO_S) {
+      cs.issue(b + OFF_TH, th + kk);
+      cs.issue(b + OFF_K, Kf + kk);
+    }
   };
   stage_in(kb, 0);
   cp_async_commit();
@@ -285,7 +294,7 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
   double HU = 0, HV = 0, HT = 0;
   // w at face k: c, xm, xp, ym, yp
   double w_c = 0, w_xm = 0, w_xp = 0, w_ym = 0, w_yp = 0;
-  if (act) {
+  if (DO_M && act) {
     const size_t kk = (size_t)kb * plane;
     const int im = pmod(i - 1, nx), ip = pmod(i + 1, nx), jm = pmod(j - 1, ny), jp = pmod(j + 1, ny);
     w_c = w[kk + oc];
@@ -295,7 +304,7 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
     w_yp = w[kk + (size_t)jp * nx + i];
   }
   // tendencies of cell k-1 (read one iteration before they are updated) and of face k
-  double rU = 0, rV = 0, rT = 0, rW = (act && kb >= 1) ? RW[(size_t)kb * plane + oc] : 0.0;
+  double rU = 0, rV = 0, rT = 0, rW = (DO_M && act && kb >= 1) ? RW[(size_t)kb * plane + oc] : 0.0;
 
 #pragma unroll 1
   for (int k = kb; k <= ke; k++) {
@@ -306,28 +315,34 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
     cp_async_commit();
     if (!act) continue;
     const double *__restrict__ su = sm + st * DIFF_STAGE, *__restrict__ sv = su + GS::SZ,
-                               *__restrict__ sw = su + 2 * GS::SZ, *__restrict__ sth = su + 3 * GS::SZ,
-                               *__restrict__ smu = su + 4 * GS::SZ, *__restrict__ sK = su + 5 * GS::SZ;
+                               *__restrict__ sw = su + 2 * GS::SZ, *__restrict__ smu = su + 3 * GS::SZ,
+                               *__restrict__ sth = su + OFF_TH, *__restrict__ sK = su + OFF_K;
     const size_t kk = (size_t)k * plane;
     const bool cell = k < nz && k < ke, inner = k >= 1 && k <= nz - 1;
     // tendencies this thread updates in the next iteration
     double rU_n = 0, rV_n = 0, rT_n = 0, rW_n = 0;
     if (cell) {
-      rU_n = RU[kk + oc];
-      rV_n = RV[kk + oc];
-      rT_n = RTh[kk + oc];
-      if (k + 1 <= nz - 1) rW_n = RW[kk + plane + oc];
+      if (DO_M) {
+        rU_n = RU[kk + oc];
+        rV_n = RV[kk + oc];
+        if (k + 1 <= nz - 1) rW_n = RW[kk + plane + oc];
+      }
+      if (DO_S) rT_n = RTh[kk + oc];
     }
     double u_c = 0, u_p = 0, v_c = 0, v_p = 0, mu_c = 0, mu_xm = 0, mu_xp = 0, mu_ym = 0, mu_yp = 0, K_c = 0, th_c = 0;
     if (k < nz) {
-      u_c = su[c]; u_p = su[c + 1]; v_c = sv[c]; v_p = sv[c + WS];
-      mu_c = smu[c]; mu_xm = smu[c - 1]; mu_xp = smu[c + 1]; mu_ym = smu[c - WS]; mu_yp = smu[c + WS];
-      K_c = sK[c]; th_c = sth[c];
+      if (DO_M) {
+        u_c = su[c]; u_p = su[c + 1]; v_c = sv[c]; v_p = sv[c + WS];
+        mu_c = smu[c]; mu_xm = smu[c - 1]; mu_xp = smu[c + 1]; mu_ym = smu[c - WS]; mu_yp = smu[c + WS];
+      }
+      if (DO_S) { K_c = sK[c]; th_c = sth[c]; }
     }
     // ---- face k: tau13 at (i,k) and (i+1,k), tau23 at (j,k) and (j+1,k), vertical scalar flux
     double t13 = 0, t13p = 0, t23 = 0, t23p = 0, Fz = 0;
     if (inner) {
       const double rhw = p.rhw[k];
+      if (DO_S) Fz = -0.5 * (K_m + K_c) * ((th_c - th_m) * rhw);
+      if (DO_M) {
       const double S13 = 0.5 * ((u_c - u_cm) * rhw + (w_c - w_xm) * rdx);
       const double S13p = 0.5 * ((u_p - u_pm) * rhw + (w_xp - w_c) * rdx);
       const double S23 = 0.5 * ((v_c - v_cm) * rhw + (w_c - w_ym) * rdy);
@@ -336,19 +351,31 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
       t13p = -2.0 * (0.25 * (mu_cm + mu_xpm + mu_c + mu_xp)) * S13p;
       t23 = -2.0 * (0.25 * (mu_ymm + mu_cm + mu_ym + mu_c)) * S23;
       t23p = -2.0 * (0.25 * (mu_cm + mu_ypm + mu_c + mu_yp)) * S23p;
-      Fz = -0.5 * (K_m + K_c) * ((th_c - th_m) * rhw);
+      }
     }
     // ---- finish cell k-1
     if (k - 1 >= k0) {
       const size_t am = kk - plane + oc;
       const double rdzm = p.rdz[k - 1];
-      RU[am] = rU - (HU + (t13 - t13_b) * rdzm);
-      RV[am] = rV - (HV + (t23 - t23_b) * rdzm);
-      RTh[am] = rT - (HT + (Fz - Fz_b) * rdzm);
+      if (DO_M) {
+        RU[am] = rU - (HU + (t13 - t13_b) * rdzm);
+        RV[am] = rV - (HV + (t23 - t23_b) * rdzm);
+      }
+      if (DO_S) RTh[am] = rT - (HT + (Fz - Fz_b) * rdzm);
     }
     if (!cell) continue;
     t13_b = t13; t23_b = t23; Fz_b = Fz;
     // ---- cell k
+    if (DO_S) {
+      // scalar fluxes through the x- and y-faces
+      const double th_xm = sth[c - 1], th_xp = sth[c + 1], th_ym = sth[c - WS], th_yp = sth[c + WS];
+      const double K_xm = sK[c - 1], K_xp = sK[c + 1], K_ym = sK[c - WS], K_yp = sK[c + WS];
+      const double Fx = -0.5 * (K_xm + K_c) * ((th_c - th_xm) * rdx), Fxp = -0.5 * (K_c + K_xp) * ((th_xp - th_c) * rdx);
+      const double Fy = -0.5 * (K_ym + K_c) * ((th_c - th_ym) * rdy), Fyp = -0.5 * (K_c + K_yp) * ((th_yp - th_c) * rdy);
+      HT = (Fxp - Fx) * rdx + (Fyp - Fy) * rdy;
+      K_m = K_c; th_m = th_c; rT = rT_n;
+    }
+    if (!DO_M) continue;
     const double u_m = su[c - 1], u_ym = su[c - WS], u_pym = su[c - WS + 1], u_yp = su[c + WS];
     const double v_m = sv[c - WS], v_xm = sv[c - 1], v_xmp = sv[c + WS - 1], v_xp = sv[c + 1];
     const double wt_c = sw[c], wt_xm = sw[c - 1], wt_xp = sw[c + 1], wt_ym = sw[c - WS], wt_yp = sw[c + WS];
@@ -371,19 +398,13 @@ __global__ void __launch_bounds__(NTHR, 2) k_diff_tiled(const SlowFlat p, const 
     const double t12xp = -2.0 * (0.25 * (mu_ym + mu_xpym + mu_c + mu_xp)) * S12xp;
     HU = (t11c - t11x) * rdx + (t12yp - t12) * rdy;
     HV = (t12xp - t12) * rdx + (t22c - t22y) * rdy;
-    // scalar fluxes through the x- and y-faces
-    const double th_xm = sth[c - 1], th_xp = sth[c + 1], th_ym = sth[c - WS], th_yp = sth[c + WS];
-    const double K_xm = sK[c - 1], K_xp = sK[c + 1], K_ym = sK[c - WS], K_yp = sK[c + WS];
-    const double Fx = -0.5 * (K_xm + K_c) * ((th_c - th_xm) * rdx), Fxp = -0.5 * (K_c + K_xp) * ((th_xp - th_c) * rdx);
-    const double Fy = -0.5 * (K_ym + K_c) * ((th_c - th_ym) * rdy), Fyp = -0.5 * (K_c + K_yp) * ((th_yp - th_c) * rdy);
-    HT = (Fxp - Fx) * rdx + (Fyp - Fy) * rdy;
     if (k >= 1 && k >= k0) RW[kk + oc] = rW - ((t13p - t13) * rdx + (t23p - t23) * rdy + (t33c - t33_m) * p.rhw[k]);
     // carry
     u_cm = u_c; u_pm = u_p; v_cm = v_c; v_pm = v_p;
     mu_cm = mu_c; mu_xmm = mu_xm; mu_xpm = mu_xp; mu_ymm = mu_ym; mu_ypm = mu_yp;
-    K_m = K_c; th_m = th_c; t33_m = t33c;
+    t33_m = t33c;
     w_c = wt_c; w_xm = wt_xm; w_xp = wt_xp; w_ym = wt_ym; w_yp = wt_yp;
-    rU = rU_n; rV = rV_n; rT = rT_n; rW = rW_n;
+    rU = rU_n; rV = rV_n; rW = rW_n;
   }
 }
 
@@ -564,18 +585,29 @@ void launch_visc_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st) {
   c->launches++;
 }
 
+template <int PART>
+static void launch_diff_part(const SlowFlat &p, dim3 grid, int kchunk, cudaStream_t st) {
+  const size_t smem = NSTAGE * diff_stage(PART) * sizeof(double) + ChunkSet<2, 1>::TAB * sizeof(int);
+  static bool once = false;
+  if (!once) {
+    cudaFuncSetAttribute(k_diff_tiled<PART>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    once = true;
+  }
+  k_diff_tiled<PART><<<grid, dim3(TX, TY), smem, st>>>(p, kchunk);
+}
+
 void launch_diff_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st) {
   int kchunk = 0;
   const int nch = level_chunks(c, &kchunk);
   dim3 grid((c->nx + TX - 1) / TX, (c->ny + TY - 1) / TY, nch);
-  const size_t smem = NSTAGE * DIFF_STAGE * sizeof(double) + ChunkSet<2, 1>::TAB * sizeof(int);
-  static bool once = false;
-  if (!once) {
-    cudaFuncSetAttribute(k_diff_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    once = true;
+  if (c->fz->variant & 1024) {  // developer knob: one launch per part (measured slower: 3.47 + 0.96 ms against 3.64 ms)
+    launch_diff_part<1>(p, grid, kchunk, st);
+    launch_diff_part<2>(p, grid, kchunk, st);
+    c->launches += 2;
+  } else {
+    launch_diff_part<3>(p, grid, kchunk, st);
+    c->launches++;
   }
-  k_diff_tiled<<<grid, dim3(TX, TY), smem, st>>>(p, kchunk);
-  c->launches++;
 }
 
 }  // namespace erfb
