@@ -64,6 +64,21 @@ def measured_traffic(kernel_class, config):
     return None
 
 
+def max_over_ranks(ms, dist, device):
+    """Step time of the whole job = the slowest rank's device time (all_reduce MAX); identity for one rank."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(world, cells, steps, ms):
+    """Whole-job throughput: every rank advances its own replica of `cells` cells by `steps` steps in `ms`."""
+    return world * cells * steps / (ms * 1e-3)
+
+
 class ClockSampler:
     """Samples SM clock and throttle reasons during the timed region (pynvml)."""
 
@@ -215,11 +230,8 @@ def run_ours(args):
     launches = dyc.launch_count - n0
     kt = dyc.timing()
     dyc.set_timing(False)
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    value = world * cells * args.steps / (ms * 1e-3)
+    ms = max_over_ranks(ms, dist, "cuda")
+    value = aggregate_value(world, cells, args.steps, ms)
 
     # ---- end to end: host buffers in, host buffers out, every step
     e2e_steps = max(1, min(args.steps, 3))
@@ -247,11 +259,8 @@ def run_ours(args):
     barrier()
     wall = time.perf_counter() - t0
     e2e_ms = max(e0.elapsed_time(e1), wall * 1e3)
-    if dist is not None:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    e2e_value = world * cells * e2e_steps / (e2e_ms * 1e-3)
+    e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
+    e2e_value = aggregate_value(world, cells, e2e_steps, e2e_ms)
     checksum = float(out_host[4].sum())
     assert np.isfinite(checksum), "state blew up"
 
