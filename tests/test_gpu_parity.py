@@ -290,10 +290,12 @@ def test_uses_the_caller_stream(torch, erfo, B):
 
 @pytest.mark.parametrize("cfg,kw", [(1, dict(nx=40, ny=23, nz=19)), (3, dict(nx=45, ny=20, nz=34)),
                                     (5, dict(nx=70, ny=11, nz=40)), (5, dict(nx=33, ny=9, nz=128))])
-def test_z_chunked_acoustic_kernel(torch, erfo, B, cfg, kw, monkeypatch):
-    """The opt-in z-chunked substep kernel (partitioned tridiagonal solve, k_acoustic_zc.cu) against the
-    oracle: n substeps through erf_acoustic and one full RK3 step (stage combine folded in)."""
-    monkeypatch.setenv("ERF_B200_VARIANT", "32")  # developer knob read by erf_create
+@pytest.mark.parametrize("variant", [32, 4096])
+def test_both_substep_kernels(torch, erfo, B, cfg, kw, variant, monkeypatch):
+    """The library picks the substep kernel by grid size (z-chunked partitioned solve, k_acoustic_zc.cu, on
+    grids with few columns; thread per column, k_fused_acoustic.cu, otherwise).  Force each in turn on the same
+    small cases: n substeps through erf_acoustic and two full RK3 steps (stage combine folded in)."""
+    monkeypatch.setenv("ERF_B200_VARIANT", str(variant))  # developer knob read by erf_create
     case = wl.make_case(cfg, **kw)
     nz, ny, nx = case["nz"], case["ny"], case["nx"]
     rng = np.random.default_rng(91 + cfg)
