@@ -29,9 +29,14 @@ __global__ void __launch_bounds__(256) k_prim_flat(const SlowFlat p) {
     const int im = i == 0 ? p.nx - 1 : i - 1, jm = j == 0 ? p.ny - 1 : j - 1;
     const size_t kk = (size_t)k * plane;
     p.theta[a] = Th / rc;
-    const double L = log1p((Th - p.Th0[k]) * p.rTh0[k]);
-    p.pp[a] = p.p0[k] * expm1(p.gam * L);   // p' = p0 [(Theta/Theta0)^gamma - 1]   [R:S1]
-    p.pi[a] = p.pi0[k] * exp(p.rdocv * L);  // pi = pi0 (Theta/Theta0)^(Rd/cv)
+    // x = Theta/Theta0 - 1.  gamma = 1 + Rd/cv, so with e = (1+x)^(Rd/cv) - 1 = expm1((Rd/cv) log1p(x)):
+    //   pi = pi0 (1 + e)                     pi = pi0 (Theta/Theta0)^(Rd/cv)
+    //   p' = p0 [(1+x)(1+e) - 1] = p0 (x + e + x e)   p' = p0 [(Theta/Theta0)^gamma - 1]   [R:S1]
+    // one log1p and one expm1 per cell, no cancellation (x, e are small and enter linearly)
+    const double x = (Th - p.Th0[k]) * p.rTh0[k];
+    const double e = expm1(p.rdocv * log1p(x));
+    p.pp[a] = p.p0[k] * (x + e + x * e);
+    p.pi[a] = p.pi0[k] * (1.0 + e);
     p.iT[a] = 1.0 / Th;
     p.u[a] = p.U[a] / (0.5 * (rho[kk + (size_t)j * p.nx + im] + rc));
     p.v[a] = p.V[a] / (0.5 * (rho[kk + (size_t)jm * p.nx + i] + rc));
