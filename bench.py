@@ -295,6 +295,15 @@ def run_ours(args):
                                "frac": ad["total"] * 8 * cells * args.steps / (ms * 1e-3) / 1e9 / peak},
                 "kernel_ms_per_step": {k: v[1] / args.steps for k, v in kt.items()}}
 
+    if roof is not None:
+        # the fp64 FMA peak of this device, measured by the library's DFMA micro-benchmark; the fp64-pipe
+        # utilisation of each kernel against it is in profiles/r1_ncu_full_cfg5.md (ncu sm__pipe_fp64_cycles_active)
+        try:
+            roof["fp64_peak_tflops"] = binding.erf_measure_fp64_peak()
+        except Exception as e:  # pragma: no cover
+            roof["fp64_peak_tflops"] = None
+            print(f"bench.py: fp64 peak not measured: {e}", file=sys.stderr)
+
     # ---- the oracle beside it, on a bounded sample (rank 0, N = 1 only)
     cpu = None
     if world == 1 and not args.no_cpu_baseline:

@@ -133,6 +133,11 @@ int erf_get_timing(erf_ctx *ctx, int id, long long *launches, double *total_ms);
 int erf_reset_timing(erf_ctx *ctx);
 const char *erf_timing_name(int id);
 
+/* The fp64 FMA peak of the current device, measured with a register-resident DFMA kernel (8 independent chains
+ * per thread, best of 3 timed launches on cuda_stream; synchronises).  *tflops counts an FMA as 2 flop.  This is the
+ * denominator for the fp64-pipe utilisation of the slow right-hand-side kernels. */
+int erf_measure_fp64_peak(double *tflops, void *cuda_stream);
+
 /* Device bytes owned by the context. */
 long long erf_device_bytes(const erf_ctx *ctx);
 

@@ -22,7 +22,8 @@ ERF_PATH_AUTO, ERF_PATH_GENERAL = 0, 1
 
 EXPORTS = ["erf_create", "erf_set_state", "erf_rk3_step", "erf_get_state", "erf_destroy",
            "erf_strerror", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_launch_count",
-           "erf_device_bytes", "erf_set_timing", "erf_get_timing", "erf_reset_timing", "erf_timing_name"]
+           "erf_device_bytes", "erf_set_timing", "erf_get_timing", "erf_reset_timing", "erf_timing_name",
+           "erf_measure_fp64_peak"]
 ERF_TIMING_CLASSES = 8
 
 _dp = C.c_void_p
@@ -88,6 +89,7 @@ def load(path: str | None = None):
     L.erf_get_timing.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_longlong), C.POINTER(C.c_double)]
     L.erf_timing_name.argtypes = [C.c_int]
     L.erf_timing_name.restype = C.c_char_p
+    L.erf_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), C.c_void_p]
     _lib = L
     return L
 
@@ -162,6 +164,13 @@ def erf_launch_count(h):
 
 def erf_device_bytes(h):
     return int(load().erf_device_bytes(h))
+
+
+def erf_measure_fp64_peak(stream=None):
+    """Measured fp64 FMA peak of the current device in TFLOP/s (FMA = 2 flop)."""
+    v = C.c_double(0.0)
+    _ck(load().erf_measure_fp64_peak(C.byref(v), _stream(stream)), "erf_measure_fp64_peak")
+    return v.value
 
 
 def erf_set_timing(h, on):

@@ -318,3 +318,9 @@ def test_both_substep_kernels(torch, erfo, B, cfg, kw, variant, monkeypatch):
     ref = _run_oracle(erfo, case, 2)
     got = _run_gpu(torch, B, case, 2)
     assert max(field_errors(got, ref)) <= TOL_1STEP * 2, field_errors(got, ref)
+
+
+def test_fp64_peak_microbenchmark(torch, B):
+    """erf_measure_fp64_peak: a plausible fp64 FMA rate for a data-centre GPU (B200: about 37 TFLOP/s)."""
+    t = B.erf_measure_fp64_peak()
+    assert 1.0 < t < 100.0, t
