@@ -24,7 +24,11 @@ using GS = TileG<2, 1>;  // halo 1 (x padded to 2)
 // ------------------------------------------------------------------ advection + PG + buoyancy
 constexpr int NSTAGE = 3;                            // pipeline depth: level k in use, k+1 and k+2 in flight
 // doubles per pipeline stage: one halo-3 tile per advected field of the launch, then the U, V, W, p' tiles
-__host__ __device__ constexpr int adv_stage(int fm) { return ((fm & 1) + ((fm >> 1) & 1) + ((fm >> 2) & 1) + ((fm >> 3) & 1)) * GB::SZ + 4 * GS::SZ; }
+// (W tile only with U or V, p' tile with U, V or W)
+__host__ __device__ constexpr int adv_stage(int fm) {
+  return ((fm & 1) + ((fm >> 1) & 1) + ((fm >> 2) & 1) + ((fm >> 3) & 1)) * GB::SZ +
+         (2 + ((fm & 6) ? 1 : 0) + ((fm & 14) ? 1 : 0)) * GS::SZ;
+}
 
 // FM = field mask: which tendencies this launch computes.  One launch with all four bits computes everything;
 // splitting by field trades re-reading the mass-flux tiles for much lower register pressure per launch.
@@ -35,6 +39,7 @@ __global__ void __launch_bounds__(NTHR, FM == F_ALL ? 2 : 3) k_adv_tiled(const S
   constexpr bool DO_T = (FM & F_T) != 0, DO_U = (FM & F_U) != 0, DO_V = (FM & F_V) != 0, DO_W = (FM & F_W) != 0;
   constexpr int ADV_STAGE = adv_stage(FM);
   constexpr int OFF_U = DO_T * GB::SZ, OFF_V = OFF_U + DO_U * GB::SZ, OFF_W = OFF_V + DO_V * GB::SZ, OFF_S = OFF_W + DO_W * GB::SZ;
+  constexpr int OFF_MW = OFF_S + 2 * GS::SZ, OFF_MP = OFF_MW + ((DO_U || DO_V) ? GS::SZ : 0);
   extern __shared__ __align__(16) double sm[];
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * TX + tx;
   const int nx = p.nx, ny = p.ny, nz = p.nz, ov = p.ov;
@@ -65,8 +70,8 @@ __global__ void __launch_bounds__(NTHR, FM == F_ALL ? 2 : 3) k_adv_tiled(const S
     double *s = b + OFF_S;
     cs.issue(s, U + kk);
     cs.issue(s + GS::SZ, V + kk);
-    if (DO_U || DO_V) cs.issue(s + 2 * GS::SZ, W + kk);
-    if (DO_U || DO_V || DO_W) cs.issue(s + 3 * GS::SZ, pp + kk);
+    if (DO_U || DO_V) cs.issue(b + OFF_MW, W + kk);
+    if (DO_U || DO_V || DO_W) cs.issue(b + OFF_MP, pp + kk);
   };
   stage_in(kb, 0);
   cp_async_commit();
@@ -113,7 +118,7 @@ __global__ void __launch_bounds__(NTHR, FM == F_ALL ? 2 : 3) k_adv_tiled(const S
     const double *__restrict__ sT = sm + st * ADV_STAGE, *__restrict__ sU = sT + OFF_U,
                                *__restrict__ sV = sT + OFF_V, *__restrict__ sW = sT + OFF_W;
     const double *__restrict__ mU = sT + OFF_S, *__restrict__ mV = mU + GS::SZ,
-                               *__restrict__ mW = mU + 2 * GS::SZ, *__restrict__ mP = mU + 3 * GS::SZ;
+                               *__restrict__ mW = sT + OFF_MW, *__restrict__ mP = sT + OFF_MP;
     const size_t kk = (size_t)k * plane;
     // own-column values for the next iteration (window tops, Omega at face k+2, rho at cell k+1)
     double nt = 0.0, nu_ = 0.0, nv = 0.0, nw = 0.0, om_nn = 0.0, rho_nn = 0.0;
