@@ -52,8 +52,8 @@ __global__ void __launch_bounds__(NTHR, FM == F_ALL ? 2 : 3) k_adv_tiled(const S
   const int ke = k1;                                              // last iteration: finishes cell k1-1
   const int kl = min(ke, nz - 1);                                 // last plane that is staged
 
-  ChunkSet<4, 3> cb;
-  ChunkSet<2, 1> cs;
+  ChunkSet<4, 3, FM != F_ALL> cb;
+  ChunkSet<2, 1, FM != F_ALL> cs;
   int *tabs = reinterpret_cast<int *>(sm + NSTAGE * ADV_STAGE);
   cb.init(tabs, tid, x0, y0, nx, ny);
   cs.init(tabs + ChunkSet<4, 3>::TAB, tid, x0, y0, nx, ny);

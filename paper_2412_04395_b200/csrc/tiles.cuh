@@ -44,28 +44,33 @@ struct TileG {
 // One thread's share of a tile copy (the same for every field with this geometry and every level).  The
 // source/destination offsets live in shared memory ([3*PER][NTHR] ints at `tab`, each thread reads only its
 // own column), not in registers: the column kernels need every register for their stencil windows.
-template <int HXP, int HY>
+template <int HXP, int HY, bool REGS = false>
 struct ChunkSet {
   using G = TileG<HXP, HY>;
   static constexpr int TAB = 3 * G::PER * NTHR;  // ints of shared memory
   const int *t;  // tab + tid
+  // REGS: when every chunk is one aligned 16-byte copy (nx even), its two offsets are kept in registers instead
+  // (kernels with registers to spare: saves three shared-memory loads and a branch per copy)
+  int rg0[REGS ? G::PER : 1], rso[REGS ? G::PER : 1];
+  bool fast;
   // g0 = offset of the chunk's first double within a plane (-1: the thread has no such chunk); g1 = offset of
   // the second double (-1: both are moved by one 16-byte copy); s = offset within the tile
   __device__ __forceinline__ void init(int *tab, int tid, int x0, int y0, int nx, int ny) {
+    fast = REGS && !(nx & 1);
 #pragma unroll
     for (int n = 0; n < G::PER; n++) {
-      const int c = tid + n * NTHR;
-      int g0 = -1, g1 = -1, so = 0;
-      if (c < G::NCH) {
-        const int ry = c / G::CW, cx = c - ry * G::CW;
-        const int gy = pmod(y0 - HY + ry, ny);
-        const int gxa = pmod(x0 - HXP + 2 * cx, nx), gxb = pmod(x0 - HXP + 2 * cx + 1, nx);
-        g0 = gy * nx + gxa;
-        const bool vec = !(nx & 1) && !(gxa & 1) && gxb == gxa + 1;
-        g1 = vec ? -1 : gy * nx + gxb;
-        so = ry * G::W + 2 * cx;
-      }
-      tab[(3 * n) * NTHR + tid] = g0;
+      // a thread without an n-th chunk repeats the copy of chunk n of thread 0 (harmless, keeps issue() branch-free)
+      const int c = tid + n * NTHR < G::NCH ? tid + n * NTHR : n * NTHR;
+      const bool have = tid + n * NTHR < G::NCH;
+      const int ry = c / G::CW, cx = c - ry * G::CW;
+      const int gy = pmod(y0 - HY + ry, ny);
+      const int gxa = pmod(x0 - HXP + 2 * cx, nx), gxb = pmod(x0 - HXP + 2 * cx + 1, nx);
+      const int g0 = gy * nx + gxa;
+      const bool vec = !(nx & 1) && !(gxa & 1) && gxb == gxa + 1;
+      const int g1 = vec ? -1 : gy * nx + gxb;
+      const int so = ry * G::W + 2 * cx;
+      if (REGS) { rg0[n] = g0; rso[n] = so; }
+      tab[(3 * n) * NTHR + tid] = have ? g0 : -1;
       tab[(3 * n + 1) * NTHR + tid] = g1;
       tab[(3 * n + 2) * NTHR + tid] = so;
     }
@@ -73,6 +78,11 @@ struct ChunkSet {
   }
   // copy this thread's chunks of one field plane (gplane = field + k * plane) into a tile
   __device__ __forceinline__ void issue(double *tile, const double *__restrict__ gplane) const {
+    if (REGS && fast) {
+#pragma unroll
+      for (int n = 0; n < G::PER; n++) cp_async16(tile + rso[n], gplane + rg0[n]);
+      return;
+    }
 #pragma unroll
     for (int n = 0; n < G::PER; n++) {
       const int g0 = t[(3 * n) * NTHR], g1 = t[(3 * n + 1) * NTHR], so = t[(3 * n + 2) * NTHR];
