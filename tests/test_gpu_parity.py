@@ -165,6 +165,21 @@ def test_full_step_count_on_crop(torch, erfo, B, cfg, kw, steps):
     assert max(field_errors(got, ref)) <= min(tol, TOL_100STEP), field_errors(got, ref)
 
 
+@pytest.mark.parametrize("cfg,kw,steps", [
+    (3, dict(nx=32, ny=24, nz=128), 100),
+    (5, dict(nx=32, ny=32, nz=128), 20),
+])
+def test_full_step_count_on_crop_thread_per_column_kernel(torch, erfo, B, cfg, kw, steps, monkeypatch):
+    """The crops above are small enough for the library to pick the z-chunked substep kernel; the kernel that runs
+    at full size (thread per column) gets the same long runs here."""
+    monkeypatch.setenv("ERF_B200_VARIANT", "4096")
+    case = wl.make_case(cfg, **kw)
+    ref = _run_oracle(erfo, case, steps)
+    got = _run_gpu(torch, B, case, steps)
+    tol = TOL_1STEP * steps if steps < 100 else TOL_100STEP
+    assert max(field_errors(got, ref)) <= min(tol, TOL_100STEP), field_errors(got, ref)
+
+
 # domain of dependence of one RK3 step in cells: 3 slow evaluations (advection +-3, plus the
 # Smagorinsky/stress stencil) and 1 + ns/2 + ns substeps of +-1 each
 def _margin(ns):
