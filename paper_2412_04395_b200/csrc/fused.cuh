@@ -27,10 +27,10 @@ struct FusedState {
   LevelTables tab;
   double *iT;         // 1/Theta^t (stage constant)
   double *U2, *V2;    // second buffers of U'', V'' (ping-pong across substeps)
-  double *Thd[2];     // Theta''_d ping-pong
-  double *cp_scr;     // Thomas c' scratch when it does not fit in shared memory
+  double *Thd[2];     // with P.Theta the three rotating Theta'' buffers (current, previous, next)
+  double *cp_scr;     // Thomas c' of the thread-per-column substep kernel (stage constant)
   double *mu, *Kd;    // dynamic viscosity and scalar diffusivity at cell centres (diffusion != 0)
-  int variant;        // tuning knob (erf_set_option)
+  int variant;        // developer knobs from the environment variable ERF_B200_VARIANT (0 = defaults)
 };
 
 int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st);

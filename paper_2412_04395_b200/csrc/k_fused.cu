@@ -42,7 +42,10 @@ int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
   memset(z, 0, sizeof(*z));
   c->fz = z;
   z->ok = c->v.flat && m->base_is_1d && c->p.substep_mode == 1;
-  if (const char *e = getenv("ERF_B200_VARIANT")) z->variant = atoi(e);  // developer tuning knob
+  // developer knobs (bit mask; 0 = the defaults bench.py times): 16 = 32-column CTAs in the z-chunked substep kernel;
+  // 32 / 4096 = force the z-chunked / the thread-per-column substep kernel; 64, 128, 192 = advection in one, two,
+  // four launches instead of three; 1024 = momentum and scalar diffusion in separate launches
+  if (const char *e = getenv("ERF_B200_VARIANT")) z->variant = atoi(e);
   if (!z->ok) return ERF_OK;
   const int nl = c->nz + 1;
   double *t[10];
