@@ -86,6 +86,7 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   c->zl_dev = nullptr;
   c->timing = false;
   c->fz = nullptr;
+  c->terr_U2 = c->terr_V2 = c->terr_rdzc = nullptr;
   for (int i = 0; i < ERF_TIMING_CLASSES; i++) { c->t_calls[i] = 0; c->t_ms[i] = 0.0; }
   memset(&c->diff, 0, sizeof(c->diff));
   memset(&c->ac, 0, sizeof(c->ac));
@@ -285,7 +286,8 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
       }
       {
         Timed t(c, T_ACOUSTIC_GENERAL, st);
-        general_acoustic(c, c->St, dtau, nsub, st);
+        if (c->path == ERF_PATH_AUTO && terrain_acoustic_available(c)) terrain_acoustic(c, c->St, dtau, nsub, st);
+        else general_acoustic(c, c->St, dtau, nsub, st);
       }
       {
         Timed t(c, T_STAGE_GENERAL, st);
@@ -335,6 +337,7 @@ extern "C" int erf_acoustic(erf_ctx *c, double dtau, int n, const double *R_rho,
     cudaMemcpyAsync(c->P.f[f], Pio[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
   }
   if (use_fused(c)) fused_acoustic(c, c->S, dtau, n, st);
+  else if (c->path == ERF_PATH_AUTO && terrain_acoustic_available(c)) terrain_acoustic(c, c->S, dtau, n, st);
   else general_acoustic(c, c->S, dtau, n, st);
   for (int f = 0; f < 5; f++)
     cudaMemcpyAsync(Pio[f], c->P.f[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);

@@ -42,6 +42,7 @@ struct erf_ctx {
   bool diff_alloc;
   erfb::gen::Acou ac;
   erfb::FusedState *fz;  // fused flat-grid path (null until fused_setup)
+  double *terr_U2, *terr_V2, *terr_rdzc;  // fused terrain substep kernel (k_acoustic_terrain.cu), allocated at first use
 
   // per-kernel timing (erf_set_timing)
   bool timing;
@@ -137,5 +138,9 @@ void general_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t
 void general_stage_init(erf_ctx *c, cudaStream_t st);    // P = S - St
 void general_stage_finish(erf_ctx *c, cudaStream_t st);  // St += P, lids
 void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st);
+
+// k_acoustic_terrain.cu: general_acoustic with the per-substep passes fused (terrain grids)
+bool terrain_acoustic_available(const erf_ctx *c);
+void terrain_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st);
 
 }  // namespace erfb
