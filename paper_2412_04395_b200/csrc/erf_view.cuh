@@ -37,9 +37,16 @@ struct View {
   const double *rho0, *Th0, *p0, *pi0;
 };
 
+// periodic wrap; offsets are at most a few cells, so one add or subtract almost always does (the modulo only
+// runs on grids narrower than the stencil)
 ERF_HD int wrapi(int a, int n) {
-  while (a < 0) a += n;
-  while (a >= n) a -= n;
+  if (a < 0) {
+    a += n;
+    if (a < 0) a = (a % n + n) % n;
+  } else if (a >= n) {
+    a -= n;
+    if (a >= n) a %= n;
+  }
   return a;
 }
 
