@@ -144,18 +144,15 @@ ERF_HD int vertical_order(int requested, int r) {  // [R:G13]
 ERF_HD double sgn_of(double m) { return m < 0.0 ? -1.0 : 1.0; }  // [R:G19]
 
 ERF_HD double interp_x(const View &c, const double *f, int m, int j, int k, int order, double M) {
-  // fixed trip count and predicated loads: q stays in registers (a run-time range would put it in local memory)
-  double q[6];
-  const int half = (order + 1) / 2;
-#pragma unroll
-  for (int n = 0; n < 6; n++) q[n] = (n >= 3 - half && n < 3 + half) ? f[IX(c, m - 3 + n, j, k)] : 0.0;
+  double q[6] = {0, 0, 0, 0, 0, 0};
+  int half = (order + 1) / 2;
+  for (int n = 3 - half; n < 3 + half; n++) q[n] = f[IX(c, m - 3 + n, j, k)];
   return interp6(order, sgn_of(M), q);
 }
 ERF_HD double interp_y(const View &c, const double *f, int i, int m, int k, int order, double M) {
-  double q[6];
-  const int half = (order + 1) / 2;
-#pragma unroll
-  for (int n = 0; n < 6; n++) q[n] = (n >= 3 - half && n < 3 + half) ? f[IX(c, i, m - 3 + n, k)] : 0.0;
+  double q[6] = {0, 0, 0, 0, 0, 0};
+  int half = (order + 1) / 2;
+  for (int n = 3 - half; n < 3 + half; n++) q[n] = f[IX(c, i, m - 3 + n, k)];
   return interp6(order, sgn_of(M), q);
 }
 // between levels m-1 and m; valid levels lo..hi
@@ -164,10 +161,9 @@ ERF_HD double interp_z(const View &c, const double *f, int i, int j, int m, int 
   int below = m - lo, above = hi - m + 1;
   int r = below < above ? below : above;
   int order = vertical_order(order_req, r);
-  const int half = (order + 1) / 2;
-  double q[6];
-#pragma unroll
-  for (int n = 0; n < 6; n++) q[n] = (n >= 3 - half && n < 3 + half) ? f[IX(c, i, j, m - 3 + n)] : 0.0;
+  int half = (order + 1) / 2;
+  double q[6] = {0, 0, 0, 0, 0, 0};
+  for (int n = 3 - half; n < 3 + half; n++) q[n] = f[IX(c, i, j, m - 3 + n)];
   return interp6(order, sgn_of(M), q);
 }
 
