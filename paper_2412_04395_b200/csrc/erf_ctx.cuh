@@ -60,39 +60,33 @@ struct erf_ctx {
 #else
 namespace erfb {
 
+// thread (i, j, k) from a 3-D launch: 32 x 8 threads over (x, y), one level per blockIdx.z (no index divisions)
 template <class F>
 __global__ void k_cells(int nx, int ny, int nlev, F f) {
-  size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  size_t n = (size_t)nx * ny * nlev;
-  if (idx >= n) return;
-  int i = (int)(idx % nx);
-  size_t r = idx / nx;
-  int j = (int)(r % ny);
-  int k = (int)(r / ny);
+  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k = blockIdx.z;
+  if (i >= nx || j >= ny || k >= nlev) return;
   f(i, j, k);
 }
 
 template <class F>
 __global__ void k_columns(int nx, int ny, F f) {
-  size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= (size_t)nx * ny) return;
-  f((int)(idx % nx), (int)(idx / nx));
+  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y;
+  if (i >= nx || j >= ny) return;
+  f(i, j);
 }
 
 template <class F>
 inline void launch_cells(erf_ctx *c, cudaStream_t st, int nlev, F f) {
-  size_t n = (size_t)c->nx * c->ny * nlev;
-  if (n == 0) return;
-  unsigned blocks = (unsigned)((n + 255) / 256);
-  k_cells<<<blocks, 256, 0, st>>>(c->nx, c->ny, nlev, f);
+  if (nlev <= 0) return;
+  dim3 block(32, 8), grid((c->nx + 31) / 32, (c->ny + 7) / 8, nlev);
+  k_cells<<<grid, block, 0, st>>>(c->nx, c->ny, nlev, f);
   c->launches++;
 }
 
 template <class F>
 inline void launch_columns(erf_ctx *c, cudaStream_t st, F f) {
-  size_t n = (size_t)c->nx * c->ny;
-  unsigned blocks = (unsigned)((n + 127) / 128);
-  k_columns<<<blocks, 128, 0, st>>>(c->nx, c->ny, f);
+  dim3 block(32, 4), grid((c->nx + 31) / 32, (c->ny + 3) / 4);
+  k_columns<<<grid, block, 0, st>>>(c->nx, c->ny, f);
   c->launches++;
 }
 
