@@ -339,3 +339,16 @@ def test_fp64_peak_microbenchmark(torch, B):
     """erf_measure_fp64_peak: a plausible fp64 FMA rate for a data-centre GPU (B200: about 37 TFLOP/s)."""
     t = B.erf_measure_fp64_peak()
     assert 1.0 < t < 100.0, t
+
+
+@pytest.mark.parametrize("kw", [dict(nx=5, ny=3, nz=96), dict(nx=33, ny=7, nz=96), dict(nx=2, ny=2, nz=96),
+                                dict(nx=64, ny=9, nz=96)])  # full nz: the stretched levels must clear the 400 m hill
+def test_terrain_ragged_and_tiny_sizes(torch, erfo, B, kw):
+    """The terrain configuration (fused terrain substep kernel + general slow RHS) on ragged and tiny grids,
+    two steps against the oracle, and against the all-general path on the device."""
+    case = wl.make_case(4, **kw)
+    ref = _run_oracle(erfo, case, 2)
+    got = _run_gpu(torch, B, case, 2)
+    assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
+    gen = _run_gpu(torch, B, case, 2, path=1)
+    assert max(field_errors(got, gen)) <= 2 * TOL_1STEP, field_errors(got, gen)
