@@ -241,7 +241,7 @@ def run_ours(args):
     d2h = h2d
     in_dev = [dev, [torch.empty_like(d) for d in dev]]
     out_dev = [dyc.empty_state(), dyc.empty_state()]
-    out_host = [[torch.empty_like(h).pin_memory() for h in host] for _ in range(2)]
+    out_host = [torch.empty_like(h).pin_memory() for h in host]  # the copies out are serialised on one stream
     s_in, s_c, s_out = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
     ev_in = [torch.cuda.Event() for _ in range(2)]    # inputs of buffer b are on the device
     ev_set = [torch.cuda.Event() for _ in range(2)]   # the library has copied buffer b in: it may be overwritten
@@ -268,7 +268,7 @@ def run_ours(args):
                 ev_c[b].record(s_c)
             with torch.cuda.stream(s_out):
                 s_out.wait_event(ev_c[b])
-                for h, d in zip(out_host[b], out_dev[b]):
+                for h, d in zip(out_host, out_dev[b]):
                     h.copy_(d, non_blocking=True)
                 ev_out[b].record(s_out)
         cur = torch.cuda.current_stream()
@@ -286,7 +286,7 @@ def run_ours(args):
     e2e_ms = max(e0.elapsed_time(e1), wall * 1e3)
     e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
     e2e_value = aggregate_value(world, cells, e2e_steps, e2e_ms)
-    checksum = float(out_host[(e2e_steps - 1) & 1][4].sum())
+    checksum = float(out_host[4].sum())
     assert np.isfinite(checksum), "state blew up"
 
     if rank != 0:
