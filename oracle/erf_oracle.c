@@ -14,7 +14,12 @@
  * (Eq. 11-13), rest state, mass / rho*theta conservation, free-stream
  * preservation over terrain, discrete acoustic dispersion (horizontal and
  * vertical), gravity-wave frequency, column solve against a dense coupled
- * solve of Appendix A, Smagorinsky closed forms, substep schedule.
+ * solve of Appendix A, Smagorinsky closed forms, substep schedule;
+ * tests/test_oracle_pins_r2.py: sign and factor of every stress component
+ * and of the scalar diffusion flux on single Fourier / cosine modes (Eq. 2-3,
+ * Eq. 9), mu = rho*nu with edge means, K = mu_t/Pr_t, the divergence-damping
+ * recurrence (L144), kinematic lids over terrain, chain-rule metric terms of
+ * the strain and of the scalar flux on Cartesian-linear fields.
  * The full nonlinear step on the benchmark configurations has no value
  * printed in the paper: "parity unpinned" beyond those invariants.
  *
