@@ -36,7 +36,7 @@ extern "C" {
 #endif
 
 #define ERF_OK 0
-#define ERF_EINVAL (-1)       /* null pointer, non-positive size, bad order / substep count / dt */
+#define ERF_EINVAL (-1)       /* null pointer, non-positive size, bad order / substep count / dt / option */
 #define ERF_EUNSUPPORTED (-2) /* non-periodic lateral boundary                                   */
 #define ERF_ENOMEM (-3)       /* host or device allocation failed                                */
 #define ERF_ECUDA (-4)        /* a CUDA runtime call or kernel launch failed (sticky)            */
@@ -74,7 +74,12 @@ typedef struct {
 } erf_params;
 
 /* Build a context: copies grid/params, derives all metric terms from the node heights
- * (S0), the base-state p0 and pi0 from Eq. 7, allocates every work array.
+ * (S0), the base-state p0 and pi0 from Eq. 7, allocates the work arrays of the path
+ * that will run (flat grid with a 1-D base state: per-level tables and the fused kernels'
+ * arrays; the terrain-general arrays are allocated on first use of that path).
+ * Any nz >= 1 is accepted with any advection order: next to the lids the vertical stencil
+ * falls back to the widest order of the same family that fits (reading G13), so a
+ * grid with fewer levels than the stencil is wide simply runs at lower vertical order.
  * The metrics pointers are read during the call only.  Synchronises cuda_stream. */
 int erf_create(const erf_grid *grid, const erf_metrics *metrics, const erf_params *params,
                void *cuda_stream, erf_ctx **out);
@@ -112,12 +117,34 @@ int erf_acoustic(erf_ctx *ctx, double dtau, int n, const double *R_rho, const do
                  const double *R_V, const double *R_W, const double *R_Theta, double *rho_pp,
                  double *U_pp, double *V_pp, double *W_pp, double *Theta_pp, void *cuda_stream);
 
+/* =====================================================================================
+ * DIAGNOSTICS -- not part of the five-call boundary; used by tests/ and bench.py only.
+ * Nothing here changes what a step computes; options select between kernels that compute
+ * the same discrete operators.
+ * ===================================================================================== */
+
 /* Select the kernel path: ERF_PATH_AUTO picks the fused kernels where they apply;
  * ERF_PATH_GENERAL forces the unfused, terrain-general kernels (one kernel per operator,
  * every intermediate field in HBM), kept as an on-device cross-check of the fused ones. */
 #define ERF_PATH_AUTO 0
 #define ERF_PATH_GENERAL 1
 int erf_set_path(erf_ctx *ctx, int path);
+
+/* erf_set_option(ctx, key, value): explicit, per-context replacements of what used to be a
+ * process-wide environment variable.  Unknown key or value: ERF_EINVAL.
+ *   ERF_OPT_VARIANT  value = OR of ERF_VARIANT_* bits, 0 = the defaults that bench.py times.
+ *   ERF_OPT_GRAPH    value = 1: erf_rk3_step captures the launches of a step into a CUDA graph
+ *                    on first use (per (dt, n_acoustic)) and replays it; 0 (default) = plain
+ *                    stream launches.  Meant for grids so small that a step is launch-bound. */
+#define ERF_OPT_VARIANT 1
+#define ERF_OPT_GRAPH 2
+#define ERF_VARIANT_ZC_WIDE 16          /* z-chunked substep kernel: 32-column CTAs            */
+#define ERF_VARIANT_FORCE_ZC 32         /* z-chunked substep kernel on every flat grid         */
+#define ERF_VARIANT_ADV_SPLIT_MASK 192  /* legacy advection: 64 one, 128 two, 192 four launches */
+#define ERF_VARIANT_DIFF_SPLIT 1024     /* momentum and scalar diffusion in separate launches  */
+#define ERF_VARIANT_FORCE_COLUMN 4096   /* thread-per-column substep kernel on every flat grid */
+#define ERF_VARIANT_SPLIT_SLOW_RHS 8192 /* round-1 slow RHS: k_prim_flat + per-field advection */
+int erf_set_option(erf_ctx *ctx, int key, long long value);
 
 /* Number of kernels launched by this context so far (for bench.py's gpu_launches). */
 long long erf_launch_count(const erf_ctx *ctx);

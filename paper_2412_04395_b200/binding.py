@@ -19,9 +19,13 @@ LIB_PATH = os.path.join(_HERE, "liberf_b200.so")
 
 ERF_OK, ERF_EINVAL, ERF_EUNSUPPORTED, ERF_ENOMEM, ERF_ECUDA = 0, -1, -2, -3, -4
 ERF_PATH_AUTO, ERF_PATH_GENERAL = 0, 1
+# erf_set_option keys and ERF_OPT_VARIANT bits (include/erf_b200.h, diagnostics block)
+ERF_OPT_VARIANT, ERF_OPT_GRAPH = 1, 2
+ERF_VARIANT_ZC_WIDE, ERF_VARIANT_FORCE_ZC, ERF_VARIANT_DIFF_SPLIT = 16, 32, 1024
+ERF_VARIANT_FORCE_COLUMN, ERF_VARIANT_SPLIT_SLOW_RHS = 4096, 8192
 
 EXPORTS = ["erf_create", "erf_set_state", "erf_rk3_step", "erf_get_state", "erf_destroy",
-           "erf_strerror", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_launch_count",
+           "erf_strerror", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_set_option", "erf_launch_count",
            "erf_device_bytes", "erf_set_timing", "erf_get_timing", "erf_reset_timing", "erf_timing_name",
            "erf_measure_fp64_peak"]
 ERF_TIMING_CLASSES = 8
@@ -80,6 +84,7 @@ def load(path: str | None = None):
     L.erf_slow_rhs.argtypes = [C.c_void_p] + [_dp] * 5 + [C.c_void_p]
     L.erf_acoustic.argtypes = [C.c_void_p, C.c_double, C.c_int] + [_dp] * 10 + [C.c_void_p]
     L.erf_set_path.argtypes = [C.c_void_p, C.c_int]
+    L.erf_set_option.argtypes = [C.c_void_p, C.c_int, C.c_longlong]
     L.erf_launch_count.argtypes = [C.c_void_p]
     L.erf_launch_count.restype = C.c_longlong
     L.erf_device_bytes.argtypes = [C.c_void_p]
@@ -156,6 +161,10 @@ def erf_acoustic(h, dtau, n, R, P, stream=None):
 
 def erf_set_path(h, path):
     _ck(load().erf_set_path(h, int(path)), "erf_set_path")
+
+
+def erf_set_option(h, key, value):
+    _ck(load().erf_set_option(h, int(key), int(value)), "erf_set_option")
 
 
 def erf_launch_count(h):
@@ -284,6 +293,9 @@ class Dycore:
 
     def set_path(self, path):
         erf_set_path(self._h, path)
+
+    def set_option(self, key, value):
+        erf_set_option(self._h, key, value)
 
     def set_timing(self, on):
         erf_set_timing(self._h, on)

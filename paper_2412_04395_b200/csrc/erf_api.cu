@@ -48,10 +48,9 @@ extern "C" void erf_destroy(erf_ctx *c) {
   if (!c) return;
   cudaDeviceSynchronize();
   fused_release(c);
-#ifndef ERF_HOSTCHECK
+  for (auto &g : c->graphs) cudaGraphExecDestroy(g.exec);
   for (auto &s : c->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
   for (auto e : c->event_pool) cudaEventDestroy(e);
-#endif
   for (void *p : c->allocs) cudaFree(p);
   delete c;
 }
@@ -104,12 +103,15 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   v.alpha = p->diffusion >= 1 ? p->alpha_theta : 0.0;
   v.Cs = p->Cs; v.Prt = p->Pr_t; v.beta_s = p->beta_s; v.beta_d = p->beta_d;
 
-  double **geo[] = {&c->zxf, &c->zyf, &c->zw, &c->hx, &c->hy, &c->hc, &c->zc, &c->hw, &c->hu, &c->hv,
-                    &c->sxw, &c->syw, &c->sxu, &c->syv, &c->rho0, &c->Th0, &c->p0, &c->pi0,
-                    &c->theta_t, &c->pi_t, &c->prim.theta, &c->prim.pp, &c->prim.pi, &c->prim.u,
-                    &c->prim.v, &c->prim.w, &c->Om_slow, &c->ac.Om, &c->ac.Th_prev, &c->ac.Thd,
-                    &c->ac.om, &c->ac.Ttil, &c->ac.rtil, &c->ac.cpr, &c->ac.dpr};
-  for (auto pp : geo) *pp = c->alloc(c->NW);
+  c->gen_ready = false;
+  c->graph_on = false;
+  c->graph_warm = false;
+  c->base1d_r0 = c->base1d_T0 = nullptr;
+  c->zxf = c->zyf = c->zw = c->hx = c->hy = c->hc = c->zc = c->hw = c->hu = c->hv = nullptr;
+  c->sxw = c->syw = c->sxu = c->syv = c->rho0 = c->Th0 = c->p0 = c->pi0 = c->Om_slow = nullptr;
+  memset(&c->prim, 0, sizeof(c->prim));
+  c->theta_t = c->alloc(c->NW);
+  c->pi_t = c->alloc(c->NW);
   for (int f = 0; f < 5; f++) {
     c->S.f[f] = c->alloc(c->NW);
     c->St.f[f] = c->alloc(c->NW);
@@ -121,36 +123,30 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
     erf_destroy(c);
     return rc;
   }
-  v.zw = c->zw; v.hx = c->hx; v.hy = c->hy; v.hc = c->hc; v.zc = c->zc; v.hw = c->hw;
-  v.hu = c->hu; v.hv = c->hv; v.sxw = c->sxw; v.syw = c->syw; v.sxu = c->sxu; v.syv = c->syv;
-  v.rho0 = c->rho0; v.Th0 = c->Th0; v.p0 = c->p0; v.pi0 = c->pi0;
-
-  // geometry from node heights (S0)
-  gen::NodeH Z;
-  Z.zn = m->z_nodes; Z.zl = nullptr; Z.nx = g->nx; Z.ny = g->ny;
-  if (!m->z_nodes) {
+  const bool fused_candidate = !m->z_nodes && m->base_is_1d;
+  if (fused_candidate) {
+    // flat grid, 1-D base state: keep the small inputs; the 3-D general arrays are built only if that path is used
     c->zl_dev = c->alloc(g->nz + 1);
-    if (!c->zl_dev) { int rc = c->status; erf_destroy(c); return rc; }
+    c->base1d_r0 = c->alloc(g->nz);
+    c->base1d_T0 = c->alloc(g->nz);
+    if (!c->zl_dev || !c->base1d_r0 || !c->base1d_T0) { int rc = c->status; erf_destroy(c); return rc; }
     cudaMemcpyAsync(c->zl_dev, m->z_levels, (g->nz + 1) * sizeof(double), cudaMemcpyHostToDevice, st);
-    Z.zl = c->zl_dev;
-  }
-  {
-    View vv = v;
-    double *zxf = c->zxf, *zyf = c->zyf, *zw = c->zw, *hx = c->hx, *hy = c->hy, *hc = c->hc, *zc = c->zc;
-    double *hw = c->hw, *hu = c->hu, *hv = c->hv, *sxu = c->sxu, *syv = c->syv, *sxw = c->sxw, *syw = c->syw;
-    double *rho0 = c->rho0, *Th0 = c->Th0, *p0 = c->p0, *pi0 = c->pi0;
-    const double *r0in = m->rho0, *t0in = m->rhotheta0;
-    int b1d = m->base_is_1d;
-    launch_cells(c, st, g->nz + 1, [=] __device__(int i, int j, int k) { gen::geo_faces(vv, Z, zxf, zyf, zw, i, j, k); });
-    launch_cells(c, st, g->nz, [=] __device__(int i, int j, int k) { gen::geo_cells(vv, zxf, zyf, zw, hx, hy, hc, zc, i, j, k); });
-    launch_cells(c, st, g->nz + 1, [=] __device__(int i, int j, int k) {
-      gen::geo_derived(vv, zxf, zyf, hc, zc, hw, hu, hv, sxu, syv, sxw, syw, i, j, k);
-    });
-    launch_cells(c, st, g->nz, [=] __device__(int i, int j, int k) {
-      gen::base_state(vv, r0in, t0in, b1d, rho0, Th0, p0, pi0, i, j, k);
-    });
+    cudaMemcpyAsync(c->base1d_r0, m->rho0, g->nz * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    cudaMemcpyAsync(c->base1d_T0, m->rhotheta0, g->nz * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  } else {
+    gen::NodeH Z;
+    Z.zn = m->z_nodes; Z.zl = nullptr; Z.nx = g->nx; Z.ny = g->ny;
+    if (!m->z_nodes) {
+      c->zl_dev = c->alloc(g->nz + 1);
+      if (!c->zl_dev) { int rc = c->status; erf_destroy(c); return rc; }
+      cudaMemcpyAsync(c->zl_dev, m->z_levels, (g->nz + 1) * sizeof(double), cudaMemcpyHostToDevice, st);
+      Z.zl = c->zl_dev;
+    }
+    int rc = build_general(c, Z, m->rho0, m->rhotheta0, m->base_is_1d, st);
+    if (rc != ERF_OK) { erf_destroy(c); return rc; }
   }
   int rc = fused_setup(c, m, st);
+  if (rc == ERF_OK && !fused_available(c)) rc = ensure_general(c, st);  // e.g. substep_mode 0 on a flat grid
   if (rc == ERF_OK && cudaStreamSynchronize(st) != cudaSuccess) rc = ERF_ECUDA;
   if (rc == ERF_OK) rc = check(c);
   if (rc != ERF_OK) {
@@ -172,7 +168,7 @@ extern "C" int erf_set_state(erf_ctx *c, const double *rho, const double *rhou, 
   cudaMemcpyAsync(c->S.f[VV], rhov, nc, cudaMemcpyDeviceToDevice, st);
   cudaMemcpyAsync(c->S.f[WW], rhow, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
   cudaMemcpyAsync(c->S.f[TH], rhotheta, nc, cudaMemcpyDeviceToDevice, st);
-  general_lids(c, c->S, st);
+  impose_lids(c, c->S, st);
   return check(c);
 }
 
@@ -197,7 +193,6 @@ extern "C" int erf_set_path(erf_ctx *c, int path) {
 }
 
 static void drain_timing(erf_ctx *c) {
-#ifndef ERF_HOSTCHECK
   for (auto &s : c->spans) {
     cudaEventSynchronize(s.b);
     float ms = 0.f;
@@ -209,7 +204,28 @@ static void drain_timing(erf_ctx *c) {
     c->event_pool.push_back(s.b);
   }
   c->spans.clear();
-#endif
+}
+
+extern "C" int erf_set_option(erf_ctx *c, int key, long long value) {
+  if (!c) return ERF_EINVAL;
+  if (key == ERF_OPT_VARIANT) {
+    const long long known = ERF_VARIANT_ZC_WIDE | ERF_VARIANT_FORCE_ZC | ERF_VARIANT_ADV_SPLIT_MASK |
+                            ERF_VARIANT_DIFF_SPLIT | ERF_VARIANT_FORCE_COLUMN | ERF_VARIANT_SPLIT_SLOW_RHS;
+    if (value < 0 || (value & ~known)) return ERF_EINVAL;
+    if (!c->fz) return ERF_OK;
+    if ((value & ERF_VARIANT_SPLIT_SLOW_RHS) && fused_available(c) && !ensure_prim(c, false)) return c->status;
+    c->fz->variant = (int)value;
+    for (auto &g : c->graphs) cudaGraphExecDestroy(g.exec);  // captured with the previous kernel choice
+    c->graphs.clear();
+    c->graph_warm = false;
+    return ERF_OK;
+  }
+  if (key == ERF_OPT_GRAPH) {
+    if (value != 0 && value != 1) return ERF_EINVAL;
+    c->graph_on = value == 1;
+    return ERF_OK;
+  }
+  return ERF_EINVAL;
 }
 
 extern "C" int erf_set_timing(erf_ctx *c, int on) {
@@ -252,15 +268,68 @@ static void schedule(int stage, double dt, int ns, int *nsub, double *dtau, doub
   else { *nsub = ns; *dtau = dt / ns; *dts = dt; }
 }
 
+// ERF_OPT_GRAPH: the fused step as a CUDA graph.  A step permutes the roles of the context's buffers (S^n <-> S^t,
+// the U''/V'' and Theta'' rotations), so one graph is captured per buffer configuration met (a handful) and the
+// permutation it causes is replayed on the host pointers after each launch.
+static std::vector<const void *> buffer_roles(const erf_ctx *c) {
+  std::vector<const void *> r;
+  for (int f = 0; f < 5; f++) { r.push_back(c->S.f[f]); r.push_back(c->St.f[f]); r.push_back(c->P.f[f]); }
+  fused_buffer_roles(c, r);
+  return r;
+}
+static void set_buffer_roles(erf_ctx *c, const std::vector<const void *> &r) {
+  size_t n = 0;
+  for (int f = 0; f < 5; f++) {
+    c->S.f[f] = (double *)r[n++]; c->St.f[f] = (double *)r[n++]; c->P.f[f] = (double *)r[n++];
+  }
+  fused_set_buffer_roles(c, r, n);
+}
+
+static int graph_step(erf_ctx *c, double dt, int ns, cudaStream_t st) {
+  const std::vector<const void *> now = buffer_roles(c);
+  for (auto &g : c->graphs)
+    if (g.dt == dt && g.ns == ns && g.before == now) {
+      if (cudaGraphLaunch(g.exec, st) != cudaSuccess) c->status = ERF_ECUDA;
+      set_buffer_roles(c, g.after);
+      c->launches += g.launches;
+      return check(c);
+    }
+  if (!c->graph_warm) {
+    c->graph_warm = true;
+    fused_rk3_step(c, dt, ns, st);
+    return check(c);
+  }
+  erf_ctx::StepGraph g;
+  g.before = now; g.dt = dt; g.ns = ns;
+  const long long l0 = c->launches;
+  cudaGraph_t graph = nullptr;
+  if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();  // the stream cannot be captured (legacy default stream): plain launches
+    fused_rk3_step(c, dt, ns, st);
+    return check(c);
+  }
+  fused_rk3_step(c, dt, ns, st);
+  if (cudaStreamEndCapture(st, &graph) != cudaSuccess || !graph) { c->status = ERF_ECUDA; return check(c); }
+  if (cudaGraphInstantiate(&g.exec, graph, 0) != cudaSuccess) { cudaGraphDestroy(graph); c->status = ERF_ECUDA; return check(c); }
+  cudaGraphDestroy(graph);
+  g.after = buffer_roles(c);
+  g.launches = c->launches - l0;
+  c->graphs.push_back(g);
+  if (cudaGraphLaunch(g.exec, st) != cudaSuccess) c->status = ERF_ECUDA;
+  return check(c);
+}
+
 extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream) {
   if (!c || !(dt > 0.0)) return ERF_EINVAL;
   if (c->p.substep_mode == 1 && (n_acoustic < 2 || (n_acoustic & 1))) return ERF_EINVAL;
   if (c->status != ERF_OK) return c->status;
   cudaStream_t st = (cudaStream_t)stream;
   if (use_fused(c)) {
+    if (c->graph_on && !c->timing) return graph_step(c, dt, n_acoustic, st);
     fused_rk3_step(c, dt, n_acoustic, st);
     return check(c);
   }
+  if (ensure_general(c, st) != ERF_OK) return c->status;
   for (int f = 0; f < 5; f++)  // S^t = S^n
     cudaMemcpyAsync(c->St.f[f], c->S.f[f], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
   for (int stage = 1; stage <= 3; stage++) {
@@ -278,7 +347,7 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
         for (int f = 0; f < 5; f++)
           if (f == WW || k < v.nz) St.f[f][a] = S.f[f][a] + dts * R.f[f][a];
       });
-      general_lids(c, c->St, st);
+      impose_lids(c, c->St, st);
     } else {
       {
         Timed t(c, T_STAGE_GENERAL, st);
@@ -309,7 +378,10 @@ extern "C" int erf_slow_rhs(erf_ctx *c, double *R_rho, double *R_U, double *R_V,
   if (c->status != ERF_OK) return c->status;
   cudaStream_t st = (cudaStream_t)stream;
   if (use_fused(c)) fused_slow_rhs(c, c->S, st);
-  else general_slow_rhs(c, c->S, st);
+  else {
+    if (ensure_general(c, st) != ERF_OK) return c->status;
+    general_slow_rhs(c, c->S, st);
+  }
   size_t nc = (size_t)c->nx * c->ny * c->nz * sizeof(double);
   double *out[5] = {R_rho, R_U, R_V, R_W, R_Theta};
   for (int f = 0; f < 5; f++)
@@ -329,7 +401,10 @@ extern "C" int erf_acoustic(erf_ctx *c, double dtau, int n, const double *R_rho,
   size_t nc = (size_t)c->nx * c->ny * c->nz * sizeof(double), nw = c->NW * sizeof(double);
   // stage constants theta^t, pi^t from the current state (the slow-RHS kernels produce them)
   if (use_fused(c)) fused_slow_rhs(c, c->S, st);
-  else general_slow_rhs(c, c->S, st);
+  else {
+    if (ensure_general(c, st) != ERF_OK) return c->status;
+    general_slow_rhs(c, c->S, st);
+  }
   const double *Rin[5] = {R_rho, R_U, R_V, R_W, R_Theta};
   double *Pio[5] = {rho_pp, U_pp, V_pp, W_pp, Theta_pp};
   for (int f = 0; f < 5; f++) {

@@ -44,6 +44,22 @@ struct erf_ctx {
   erfb::FusedState *fz;  // fused flat-grid path (null until fused_setup)
   double *terr_U2, *terr_V2, *terr_rdzc;  // fused terrain substep kernel (k_acoustic_terrain.cu), allocated at first use
 
+  // The terrain-general arrays (3-D metrics, base state, unfused intermediates) exist only where that path runs:
+  // always on terrain / 3-D base states, on flat grids from the first use of ERF_PATH_GENERAL (ensure_general).
+  bool gen_ready;
+  double *base1d_r0, *base1d_T0;  // flat grid, 1-D base state: owned copies of the [nz] inputs (to build the 3-D arrays later)
+
+  // ERF_OPT_GRAPH: one instantiated CUDA graph per buffer configuration of the fused step
+  struct StepGraph {
+    std::vector<const void *> before, after;  // buffer roles when the step starts / ends
+    double dt;
+    int ns;
+    long long launches;
+    cudaGraphExec_t exec;
+  };
+  bool graph_on, graph_warm;  // warm: a plain step has run (kernel attributes are set outside any capture)
+  std::vector<StepGraph> graphs;
+
   // per-kernel timing (erf_set_timing)
   bool timing;
   struct TimedSpan { int id; cudaEvent_t a, b; };
@@ -55,9 +71,6 @@ struct erf_ctx {
   double *alloc(size_t n);  // zero-initialised device doubles; null on failure (sets status)
 };
 
-#ifdef ERF_HOSTCHECK  // developer-only host emulation of the launches (never built into the library)
-#include "host_launch.h"
-#else
 namespace erfb {
 
 // thread (i, j, k) from a 3-D launch: 32 x 8 threads over (x, y), one level per blockIdx.z (no index divisions)
@@ -91,7 +104,6 @@ inline void launch_columns(erf_ctx *c, cudaStream_t st, F f) {
 }
 
 }  // namespace erfb
-#endif
 
 namespace erfb {
 
@@ -105,7 +117,6 @@ struct Timed {
   cudaStream_t st;
   int idx;
   Timed(erf_ctx *c_, int id, cudaStream_t st_) : c(c_), st(st_), idx(-1) {
-#ifndef ERF_HOSTCHECK
     if (!c->timing) return;
     erf_ctx::TimedSpan s;
     s.id = id;
@@ -117,16 +128,18 @@ struct Timed {
     cudaEventRecord(s.a, st);
     c->spans.push_back(s);
     idx = (int)c->spans.size() - 1;
-#endif
   }
   ~Timed() {
-#ifndef ERF_HOSTCHECK
     if (idx >= 0) cudaEventRecord(c->spans[idx].b, st);
-#endif
   }
 };
 
-// general path (k_general.cu)
+// general path (k_general.cu).  ensure_general allocates and fills the 3-D metric / base-state arrays and the unfused
+// intermediates on first use (returns the context status); every general_* function below requires it.
+int ensure_general(erf_ctx *c, cudaStream_t st);
+int build_general(erf_ctx *c, const gen::NodeH &Z, const double *rho0_in, const double *Th0_in, int base1d, cudaStream_t st);
+bool ensure_prim(erf_ctx *c, bool all);  // u, v, w, p' (all: also theta, pi) work arrays
+void impose_lids(erf_ctx *c, const F5 &S, cudaStream_t st);  // kinematic W on k = 0 and k = nz [R:G15]
 void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st);  // fills c->R, theta_t, pi_t
 void general_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st);  // c->P in/out
 void general_stage_init(erf_ctx *c, cudaStream_t st);    // P = S - St

@@ -4,6 +4,8 @@
 // metric term is a per-level constant (hx = hy = hc = dz(k), slopes = 0, Omega = W), so
 // the column operators read short per-level tables instead of 3-D metric fields.
 #pragma once
+#include <vector>
+
 #include "erf_ctx.cuh"
 
 namespace erfb {
@@ -30,7 +32,7 @@ struct FusedState {
   double *Thd[2];     // with P.Theta the three rotating Theta'' buffers (current, previous, next)
   double *cp_scr;     // Thomas c' of the thread-per-column substep kernel (stage constant)
   double *mu, *Kd;    // dynamic viscosity and scalar diffusivity at cell centres (diffusion != 0)
-  int variant;        // developer knobs from the environment variable ERF_B200_VARIANT (0 = defaults)
+  int variant;        // ERF_VARIANT_* mask (erf_set_option, diagnostics block of erf_b200.h); 0 = defaults
 };
 
 int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st);
@@ -39,6 +41,9 @@ bool fused_available(const erf_ctx *c);
 void fused_rk3_step(erf_ctx *c, double dt, int n_acoustic, cudaStream_t st);
 void fused_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st);
 void fused_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st);
+// the fused path's own rotating buffers, appended to / restored from the list erf_api.cu keeps per CUDA graph
+void fused_buffer_roles(const erf_ctx *c, std::vector<const void *> &r);
+void fused_set_buffer_roles(erf_ctx *c, const std::vector<const void *> &r, size_t n);
 
 // k_fused_slow.cu
 void launch_slow_flat(erf_ctx *c, const F5 &S, cudaStream_t st);

@@ -42,19 +42,44 @@ int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
   memset(z, 0, sizeof(*z));
   c->fz = z;
   z->ok = c->v.flat && m->base_is_1d && c->p.substep_mode == 1;
-  // developer knobs (bit mask; 0 = the defaults bench.py times): 16 = 32-column CTAs in the z-chunked substep kernel;
-  // 32 / 4096 = force the z-chunked / the thread-per-column substep kernel; 64, 128, 192 = advection in one, two,
-  // four launches instead of three; 1024 = momentum and scalar diffusion in separate launches
-  if (const char *e = getenv("ERF_B200_VARIANT")) z->variant = atoi(e);
+  z->variant = 0;  // kernel-variant mask, erf_set_option(ERF_OPT_VARIANT)
   if (!z->ok) return ERF_OK;
   const int nl = c->nz + 1;
+  // Per-level tables.  They come from the SAME geometry / base-state routines as the 3-D arrays of the general
+  // path, run on a one-column periodic grid (on a flat grid every column is that column), so both paths see
+  // bit-identical metric terms without the 3-D arrays ever being allocated here.
+  View vc = c->v;
+  vc.nx = vc.ny = 1;
+  double *col[18];
+  for (auto &p : col) {
+    p = c->alloc(nl);
+    if (!p) return c->status;
+  }
+  double *zxf = col[0], *zyf = col[1], *zw = col[2], *hx = col[3], *hy = col[4], *hc = col[5], *zc = col[6];
+  double *hw = col[7], *hu = col[8], *hv = col[9], *sxu = col[10], *syv = col[11], *sxw = col[12], *syw = col[13];
+  double *rho0 = col[14], *Th0 = col[15], *p0 = col[16], *pi0 = col[17];
+  vc.hc = hc; vc.hw = hw; vc.rho0 = rho0; vc.Th0 = Th0; vc.p0 = p0; vc.pi0 = pi0;
+  gen::NodeH Z;
+  Z.zn = nullptr; Z.zl = c->zl_dev; Z.nx = 1; Z.ny = 1;
+  const double *r0in = c->base1d_r0, *t0in = c->base1d_T0;
+  const int nz = c->nz;
+  View vv = vc;
+  auto column = [&](int nlev, auto f) {
+    k_cells<<<dim3(1, 1, nlev), dim3(32, 8), 0, st>>>(1, 1, nlev, f);
+    c->launches++;
+  };
+  column(nz + 1, [=] __device__(int i, int j, int k) { gen::geo_faces(vv, Z, zxf, zyf, zw, i, j, k); });
+  column(nz, [=] __device__(int i, int j, int k) { gen::geo_cells(vv, zxf, zyf, zw, hx, hy, hc, zc, i, j, k); });
+  column(nz + 1, [=] __device__(int i, int j, int k) {
+    gen::geo_derived(vv, zxf, zyf, hc, zc, hw, hu, hv, sxu, syv, sxw, syw, i, j, k);
+  });
+  column(nz, [=] __device__(int i, int j, int k) { gen::base_state(vv, r0in, t0in, 1, rho0, Th0, p0, pi0, i, j, k); });
   double *t[10];
   for (auto &p : t) {
     p = c->alloc(nl);
     if (!p) return c->status;
   }
-  k_level_tables<<<(nl + 127) / 128, 128, 0, st>>>(c->v, t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7],
-                                                       t[8], t[9]);
+  k_level_tables<<<(nl + 127) / 128, 128, 0, st>>>(vc, t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7], t[8], t[9]);
   c->launches++;
   z->tab = LevelTables{t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7], t[8], t[9]};
   double **arr[] = {&z->iT, &z->U2, &z->V2, &z->Thd[0], &z->Thd[1], &z->cp_scr};
@@ -66,8 +91,20 @@ int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
     z->mu = c->alloc(c->NW);
     z->Kd = c->alloc(c->NW);
     if (!z->mu || !z->Kd) return c->status;
+    if (!ensure_prim(c, false)) return c->status;  // u, v, w for the diffusion kernels
   }
+  if ((c->nx & 1) && !ensure_prim(c, false)) return c->status;  // odd nx: the round-1 slow-RHS kernels
   return ERF_OK;
+}
+
+void fused_buffer_roles(const erf_ctx *c, std::vector<const void *> &r) {
+  const FusedState *z = c->fz;
+  r.push_back(z->U2); r.push_back(z->V2); r.push_back(z->Thd[0]); r.push_back(z->Thd[1]);
+}
+
+void fused_set_buffer_roles(erf_ctx *c, const std::vector<const void *> &r, size_t n) {
+  FusedState *z = c->fz;
+  z->U2 = (double *)r[n]; z->V2 = (double *)r[n + 1]; z->Thd[0] = (double *)r[n + 2]; z->Thd[1] = (double *)r[n + 3];
 }
 
 void fused_release(erf_ctx *c) {

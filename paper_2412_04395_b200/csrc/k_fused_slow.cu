@@ -61,10 +61,14 @@ void launch_slow_flat(erf_ctx *c, const F5 &S, cudaStream_t st) {
   p.gam = c->v.gam; p.rdocv = c->v.rdocv; p.nu = c->v.nu; p.alpha = c->v.alpha;
   p.rPrt = c->p.diffusion == 2 ? 1.0 / c->v.Prt : 0.0;
   p.diffusion = c->p.diffusion;
-  const size_t plane = (size_t)c->nx * c->ny;
-  k_prim_flat<<<(unsigned)((plane * (c->nz + 1) + 255) / 256), 256, 0, st>>>(p);
-  c->launches++;
-  launch_adv_diff_tiled(c, p, st);
+  if (slow_adv_available(c) && !(z->variant & ERF_VARIANT_SPLIT_SLOW_RHS)) {
+    launch_slow_adv(c, p, st);
+  } else {
+    const size_t plane = (size_t)c->nx * c->ny;
+    k_prim_flat<<<(unsigned)((plane * (c->nz + 1) + 255) / 256), 256, 0, st>>>(p);
+    c->launches++;
+    launch_adv_diff_tiled(c, p, st);
+  }
   if (c->p.diffusion != 0) {
     launch_visc_tiled(c, p, st);
     launch_diff_tiled(c, p, st);

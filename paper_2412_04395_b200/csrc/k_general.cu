@@ -18,6 +18,76 @@ static bool ensure_diff(erf_ctx *c) {
   return true;
 }
 
+// u, v, w, p' (and theta, pi with `all`) work arrays: the general path and the round-1 fused slow-RHS kernels use them
+bool ensure_prim(erf_ctx *c, bool all) {
+  double **need[] = {&c->prim.u, &c->prim.v, &c->prim.w, &c->prim.pp, &c->prim.theta, &c->prim.pi};
+  for (int n = 0; n < (all ? 6 : 4); n++)
+    if (!*need[n]) {
+      *need[n] = c->alloc(c->NW);
+      if (!*need[n]) return false;
+    }
+  return true;
+}
+
+// the 3-D metric terms (S0) from the node heights, the 3-D base state with p0, pi0 from Eq. 7, and the
+// unfused path's intermediates
+int build_general(erf_ctx *c, const gen::NodeH &Z, const double *r0in, const double *t0in, int b1d, cudaStream_t st) {
+  if (c->gen_ready) return c->status;
+  double **geo[] = {&c->zxf, &c->zyf, &c->zw, &c->hx, &c->hy, &c->hc, &c->zc, &c->hw, &c->hu, &c->hv,
+                    &c->sxw, &c->syw, &c->sxu, &c->syv, &c->rho0, &c->Th0, &c->p0, &c->pi0,
+                    &c->Om_slow, &c->ac.Om, &c->ac.Th_prev, &c->ac.Thd,
+                    &c->ac.om, &c->ac.Ttil, &c->ac.rtil, &c->ac.cpr, &c->ac.dpr};
+  for (auto pp : geo) {
+    *pp = c->alloc(c->NW);
+    if (!*pp) return c->status;
+  }
+  if (!ensure_prim(c, true)) return c->status;
+  View &v = c->v;
+  v.zw = c->zw; v.hx = c->hx; v.hy = c->hy; v.hc = c->hc; v.zc = c->zc; v.hw = c->hw;
+  v.hu = c->hu; v.hv = c->hv; v.sxw = c->sxw; v.syw = c->syw; v.sxu = c->sxu; v.syv = c->syv;
+  v.rho0 = c->rho0; v.Th0 = c->Th0; v.p0 = c->p0; v.pi0 = c->pi0;
+  View vv = v;
+  double *zxf = c->zxf, *zyf = c->zyf, *zw = c->zw, *hx = c->hx, *hy = c->hy, *hc = c->hc, *zc = c->zc;
+  double *hw = c->hw, *hu = c->hu, *hv = c->hv, *sxu = c->sxu, *syv = c->syv, *sxw = c->sxw, *syw = c->syw;
+  double *rho0 = c->rho0, *Th0 = c->Th0, *p0 = c->p0, *pi0 = c->pi0;
+  const int nz = c->nz;
+  launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::geo_faces(vv, Z, zxf, zyf, zw, i, j, k); });
+  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::geo_cells(vv, zxf, zyf, zw, hx, hy, hc, zc, i, j, k); });
+  launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) {
+    gen::geo_derived(vv, zxf, zyf, hc, zc, hw, hu, hv, sxu, syv, sxw, syw, i, j, k);
+  });
+  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
+    gen::base_state(vv, r0in, t0in, b1d, rho0, Th0, p0, pi0, i, j, k);
+  });
+  c->gen_ready = true;
+  return c->status;
+}
+
+// flat grids with a 1-D base state build the general arrays only when that path is first used
+int ensure_general(erf_ctx *c, cudaStream_t st) {
+  if (c->gen_ready) return c->status;
+  if (!c->zl_dev || !c->base1d_r0) return c->status = ERF_EINVAL;
+  gen::NodeH Z;
+  Z.zn = nullptr; Z.zl = c->zl_dev; Z.nx = c->nx; Z.ny = c->ny;
+  return build_general(c, Z, c->base1d_r0, c->base1d_T0, 1, st);
+}
+
+// kinematic W on the lids [R:G15]; on a flat grid the slopes vanish identically: W = 0
+void impose_lids(erf_ctx *c, const F5 &S, cudaStream_t st) {
+  if (c->gen_ready) {
+    general_lids(c, S, st);
+    return;
+  }
+  double *W = S.f[WW];
+  const size_t plane = (size_t)c->nx * c->ny, top = plane * c->nz;
+  const int nx = c->nx;
+  launch_columns(c, st, [=] __device__(int i, int j) {
+    const size_t a = (size_t)j * nx + i;
+    W[a] = 0.0;
+    W[top + a] = 0.0;
+  });
+}
+
 void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st) {
   View v = c->v;
   const double *U = S.f[UU], *V = S.f[VV];

@@ -50,6 +50,10 @@ __device__ __forceinline__ int vorder(int req, int r) {
   return 2;
 }
 
+// k_slow_adv.cu: primitives + advection + pressure gradient + buoyancy in one kernel (needs nx even)
+bool slow_adv_available(const erf_ctx *c);
+void launch_slow_adv(erf_ctx *c, const SlowFlat &p, cudaStream_t st);
+
 // k_slow_tiled.cu
 void launch_adv_diff_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st);
 void launch_diff_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st);

@@ -44,13 +44,22 @@ def _host(ts):
     return [t.cpu().numpy() for t in ts]
 
 
-def _run_gpu(torch, B, case, steps, path=None, state=None):
+def _run_gpu(torch, B, case, steps, path=None, state=None, variant=None, graph=False):
     d = B.Dycore(case)
     if path is not None:
         d.set_path(path)
+    if variant is not None:
+        d.set_option(B.ERF_OPT_VARIANT, variant)
+    if graph:
+        d.set_option(B.ERF_OPT_GRAPH, 1)
     d.set_state(*_dev(torch, state if state is not None else case["state"]))
-    for _ in range(steps):
-        d.rk3_step(case["dt"], case["ns"])
+    torch.cuda.synchronize()
+    # graphs need a capturable stream (the legacy default stream is not)
+    side = torch.cuda.Stream() if graph else torch.cuda.current_stream()
+    with torch.cuda.stream(side):
+        for _ in range(steps):
+            d.rk3_step(case["dt"], case["ns"])
+    side.synchronize()
     out = _host(d.get_state())
     torch.cuda.synchronize()
     n = d.launch_count
@@ -69,10 +78,12 @@ def _run_oracle(erfo, case, steps, state=None):
     return out
 
 
-SMALL = [  # several tiles plus a ragged tail in every direction
+SMALL = [  # several tiles plus a ragged tail in every direction; odd nx takes the 8-byte-copy kernels
     (1, dict(nx=40, ny=23, nz=19)),
     (2, dict(nx=37, ny=18, nz=21)),
+    (2, dict(nx=38, ny=19, nz=21)),
     (3, dict(nx=45, ny=20, nz=34)),
+    (3, dict(nx=46, ny=21, nz=34)),
     (4, dict(nx=44, ny=36, nz=96)),
     (5, dict(nx=70, ny=11, nz=40)),
 ]
@@ -169,13 +180,12 @@ def test_full_step_count_on_crop(torch, erfo, B, cfg, kw, steps):
     (3, dict(nx=32, ny=24, nz=128), 100),
     (5, dict(nx=32, ny=32, nz=128), 20),
 ])
-def test_full_step_count_on_crop_thread_per_column_kernel(torch, erfo, B, cfg, kw, steps, monkeypatch):
+def test_full_step_count_on_crop_thread_per_column_kernel(torch, erfo, B, cfg, kw, steps):
     """The crops above are small enough for the library to pick the z-chunked substep kernel; the kernel that runs
     at full size (thread per column) gets the same long runs here."""
-    monkeypatch.setenv("ERF_B200_VARIANT", "4096")
     case = wl.make_case(cfg, **kw)
     ref = _run_oracle(erfo, case, steps)
-    got = _run_gpu(torch, B, case, steps)
+    got = _run_gpu(torch, B, case, steps, variant=B.ERF_VARIANT_FORCE_COLUMN)
     tol = TOL_1STEP * steps if steps < 100 else TOL_100STEP
     assert max(field_errors(got, ref)) <= min(tol, TOL_100STEP), field_errors(got, ref)
 
@@ -306,11 +316,10 @@ def test_uses_the_caller_stream(torch, erfo, B):
 @pytest.mark.parametrize("cfg,kw", [(1, dict(nx=40, ny=23, nz=19)), (3, dict(nx=45, ny=20, nz=34)),
                                     (5, dict(nx=70, ny=11, nz=40)), (5, dict(nx=33, ny=9, nz=128))])
 @pytest.mark.parametrize("variant", [32, 4096])
-def test_both_substep_kernels(torch, erfo, B, cfg, kw, variant, monkeypatch):
+def test_both_substep_kernels(torch, erfo, B, cfg, kw, variant):
     """The library picks the substep kernel by grid size (z-chunked partitioned solve, k_acoustic_zc.cu, on
     grids with few columns; thread per column, k_fused_acoustic.cu, otherwise).  Force each in turn on the same
     small cases: n substeps through erf_acoustic and two full RK3 steps (stage combine folded in)."""
-    monkeypatch.setenv("ERF_B200_VARIANT", str(variant))  # developer knob read by erf_create
     case = wl.make_case(cfg, **kw)
     nz, ny, nx = case["nz"], case["ny"], case["nx"]
     rng = np.random.default_rng(91 + cfg)
@@ -324,6 +333,7 @@ def test_both_substep_kernels(torch, erfo, B, cfg, kw, variant, monkeypatch):
     ref = o.acoustic(dtau, 4, R, P)
     o.close()
     d = B.Dycore(case)
+    d.set_option(B.ERF_OPT_VARIANT, variant)
     d.set_state(*_dev(torch, case["state"]))
     got = _host(d.acoustic(dtau, 4, _dev(torch, R), _dev(torch, P)))
     d.close()
@@ -331,8 +341,34 @@ def test_both_substep_kernels(torch, erfo, B, cfg, kw, variant, monkeypatch):
     got[3][nz] = ref[3][nz]
     assert max(field_errors(got, ref)) <= TOL_1STEP, field_errors(got, ref)
     ref = _run_oracle(erfo, case, 2)
-    got = _run_gpu(torch, B, case, 2)
+    got = _run_gpu(torch, B, case, 2, variant=variant)
     assert max(field_errors(got, ref)) <= TOL_1STEP * 2, field_errors(got, ref)
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict(nx=40, ny=24, nz=19)), (2, dict(nx=38, ny=19, nz=21)),
+                                    (3, dict(nx=46, ny=21, nz=34)), (5, dict(nx=70, ny=11, nz=40)),
+                                    (5, dict(nx=64, ny=16, nz=7)), (2, dict(nx=2, ny=2, nz=3))])
+def test_round1_slow_rhs_kernels_agree_with_the_fused_one(torch, erfo, B, cfg, kw):
+    """The single-launch primitives + advection + pressure-gradient kernel (k_slow_adv.cu, bulk-copy tiles) against the
+    round-1 kernels (k_prim_flat + per-field k_adv_tiled), which are still what odd nx runs: both against the oracle
+    after two full steps."""
+    case = wl.make_case(cfg, **kw)
+    ref = _run_oracle(erfo, case, 2)
+    new = _run_gpu(torch, B, case, 2)
+    old = _run_gpu(torch, B, case, 2, variant=B.ERF_VARIANT_SPLIT_SLOW_RHS)
+    assert max(field_errors(new, ref)) <= 2 * TOL_1STEP, field_errors(new, ref)
+    assert max(field_errors(old, ref)) <= 2 * TOL_1STEP, field_errors(old, ref)
+
+
+@pytest.mark.parametrize("cfg,kw", [(1, dict()), (2, dict(nx=64, ny=48, nz=32))])
+def test_cuda_graph_replay_is_bitwise_the_stream_launch(torch, B, cfg, kw):
+    """ERF_OPT_GRAPH: the step replayed from captured CUDA graphs (one per buffer configuration) must give the very
+    same bits as plain stream launches, over enough steps to revisit every configuration."""
+    case = wl.make_case(cfg, **kw)
+    a = _run_gpu(torch, B, case, 9)
+    b = _run_gpu(torch, B, case, 9, graph=True)
+    for x, y in zip(a, b):
+        assert np.array_equal(x, y)
 
 
 def test_fp64_peak_microbenchmark(torch, B):
