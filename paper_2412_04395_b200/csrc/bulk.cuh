@@ -1,5 +1,8 @@
-// bulk.cuh -- shared-memory plane tiles filled by the bulk-copy engine (cp.async.bulk, SASS UBLKCP) with
-// mbarrier completion (SASS SYNCS).
+// bulk.cuh -- shared-memory plane tiles filled by the bulk-copy engine with mbarrier completion (SASS SYNCS):
+// TMA tensor copies (cp.async.bulk.tensor.3d, SASS UTMALDG) -- one instruction per field and level -- for the CTAs
+// whose halo tile lies inside the domain, row-wise bulk copies (cp.async.bulk, SASS UBLKCP) with the periodic wrap
+// in the source address for the CTAs on the periodic seam (the tensor unit fills out-of-range boxes with zeros, it
+// cannot wrap).
 //
 // A tile is H rows of W doubles of one horizontal plane of a dense [.][ny][nx] field, starting at column
 // xs (even) and row ys, both taken modulo the domain: the periodic lateral boundary is a wrap of
@@ -8,6 +11,7 @@
 // multi-field stage, every thread then waits on the stage's mbarrier.  Requirements of cp.async.bulk: 16-byte
 // aligned source, destination and size -- hence nx even, xs even, W even (checked by the launchers).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cstdint>
@@ -47,6 +51,18 @@ __device__ __forceinline__ void bulk_g2s(double *dst, const double *src, unsigne
                "l"(src), "r"(bytes), "r"(smem_u32(bar))
                : "memory");
 }
+
+// whole-tile TMA copy: box (bw x bh x 1) of the 3-D tensor described by `map` with its corner at (x, y, z)
+__device__ __forceinline__ void tma_tile_g2s(double *dst, const CUtensorMap *map, int x, int y, int z, uint64_t *bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];\n" ::"r"(
+          smem_u32(dst)),
+      "l"(map), "r"(x), "r"(y), "r"(z), "r"(smem_u32(bar))
+      : "memory");
+}
+
+// host: tensor map of a dense [nlev][ny][nx] fp64 field with a (bw x bh x 1) box; false if the driver refuses
+bool make_tile_map(CUtensorMap *out, const double *base, int nx, int ny, int nlev, int bw, int bh);
 
 __device__ __forceinline__ int pmodi(int a, int n) {
   a %= n;

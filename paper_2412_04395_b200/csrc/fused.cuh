@@ -4,6 +4,9 @@
 // metric term is a per-level constant (hx = hy = hc = dz(k), slopes = 0, Omega = W), so
 // the column operators read short per-level tables instead of 3-D metric fields.
 #pragma once
+#include <cuda.h>
+
+#include <map>
 #include <vector>
 
 #include "erf_ctx.cuh"
@@ -32,6 +35,7 @@ struct FusedState {
   double *Thd[2];     // with P.Theta the three rotating Theta'' buffers (current, previous, next)
   double *cp_scr;     // Thomas c' of the thread-per-column substep kernel (stage constant)
   double *mu, *Kd;    // dynamic viscosity and scalar diffusivity at cell centres (diffusion != 0)
+  std::map<const void *, CUtensorMap> tmaps;  // TMA tensor maps of the state buffers (k_slow_adv.cu)
   int variant;        // ERF_VARIANT_* mask (erf_set_option, diagnostics block of erf_b200.h); 0 = defaults
 };
 

@@ -38,8 +38,7 @@ __global__ void k_level_tables(View v, double *dz, double *rdz, double *rhw, dou
 }
 
 int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
-  FusedState *z = new FusedState();
-  memset(z, 0, sizeof(*z));
+  FusedState *z = new FusedState();  // value-initialised: every pointer null
   c->fz = z;
   z->ok = c->v.flat && m->base_is_1d && c->p.substep_mode == 1;
   z->variant = 0;  // kernel-variant mask, erf_set_option(ERF_OPT_VARIANT)

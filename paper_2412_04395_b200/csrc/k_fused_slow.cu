@@ -61,6 +61,7 @@ void launch_slow_flat(erf_ctx *c, const F5 &S, cudaStream_t st) {
   p.gam = c->v.gam; p.rdocv = c->v.rdocv; p.nu = c->v.nu; p.alpha = c->v.alpha;
   p.rPrt = c->p.diffusion == 2 ? 1.0 / c->v.Prt : 0.0;
   p.diffusion = c->p.diffusion;
+  p.use_tma = 0;
   if (slow_adv_available(c) && !(z->variant & ERF_VARIANT_SPLIT_SLOW_RHS)) {
     launch_slow_adv(c, p, st);
   } else {

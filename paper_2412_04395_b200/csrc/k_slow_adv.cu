@@ -11,19 +11,21 @@
 //
 // Layout of the work.  A CTA owns 32 x 8 columns (and a range of levels on small grids) and marches upward.  For
 // every level the five state planes arrive as halo tiles through cp.async.bulk row copies (bulk.cuh; ring of NS
-// stages, filled two levels ahead, periodic wrap in the source address).  All 768 threads first turn the newly
+// stages, filled two levels ahead, periodic wrap in the source address).  All 512 threads first turn the newly
 // landed level into primitive tiles theta, u, v, w (halo 3) and p' (halo 1) in shared memory -- each primitive is
 // computed once per tile point instead of once per consumer -- and write theta^t, pi^t, 1/Theta^t of the interior.
-// Then three groups of 256 threads (warp-uniform roles) each handle one column per thread:
-//     group 0: rho and rho*theta,   group 1: rho*u and rho*v,   group 2: rho*w (+ vertical PG and buoyancy).
-// Splitting by field keeps every thread under 85 registers (768 threads per SM) while the tiles are loaded and the
-// primitives computed once for all three.
+// Then two groups of 256 threads (warp-uniform roles) each handle one column per thread:
+//     group 0: rho, rho*theta and rho*w (+ vertical pressure gradient and buoyancy),   group 1: rho*u and rho*v.
+// The two roles carry about the same arithmetic; splitting by field halves the per-thread state (vertical windows,
+// FIFOs) while the tiles are loaded and the primitives computed once for both.
 //
 // Vertical stencils.  The horizontal work of a thread runs at the "front" level L (the plane that is resident with
-// its halo); its horizontal divergences are parked in a three-deep FIFO (registers; shared memory for group 1).
-// The value of the own column at level L enters a six-deep register window, which is what the vertical flux at
-// face L-2 (cells L-5 .. L) needs; cell L-3 is finished in the same iteration.  So no plane other than the front
-// one is ever read, and nothing is re-loaded from global memory.
+// its halo); its horizontal divergences are parked in a three-deep register FIFO.  The value of the own column at
+// level L enters a six-deep register window, which is what the vertical flux at face L-2 (cells L-5 .. L) needs;
+// cell L-3 is finished in the same iteration.  So no plane other than the front one is ever read, and nothing is
+// re-loaded from global memory.
+#include <cstring>
+
 #include "bulk.cuh"
 #include "slow_flat.cuh"
 
@@ -32,18 +34,36 @@ namespace sadv {
 
 constexpr int TX = 32, TY = 8, HX = 4, HY = 4;
 constexpr int TW = TX + 2 * HX, TH = TY + 2 * HY, TSZ = TW * TH;  // 40 x 16 tile (rho: all rows; others rows 1..14)
-constexpr int NS = 4;                                             // raw ring: levels P-1 .. P+2
+constexpr int NS = 5;                                             // raw ring: levels P-2 .. P+2
 constexpr int NPB = 3;                                            // primitive buffers
 constexpr int PW = 36, PH = 10, PSZ = PW * PH;                    // p' tile: x in [-2, 33], y in [-1, 8]
 constexpr int RAW = 5 * TSZ, PB = 4 * TSZ + PSZ;
-constexpr int NTH = 768, NCOL = TX * TY;
+constexpr int NTH = 512, NCOL = TX * TY;
 constexpr int NCOPY = TH + 4 * (TH - 2);                          // row copies per level: 16 + 4 * 14
-constexpr size_t SMEM = (size_t)(NS * RAW + NPB * PB + NCOL * 4 * 2) * sizeof(double) + NS * sizeof(uint64_t);
+constexpr int NTAB = 8;                                           // per-level tables staged in shared memory
+constexpr int MAXLEV = 320;                                       // nz + 1 <= MAXLEV (shared-memory budget)
+constexpr size_t smem_bytes(int nlev) {
+  return (size_t)(NS * RAW + NPB * PB + NTAB * nlev) * sizeof(double) + NS * sizeof(uint64_t);
+}
+
+struct Maps {
+  CUtensorMap m[5];  // rho, U, V, W, Theta: (TW x TH x 1) boxes
+};
 
 struct Poly {
   double c[12];  // (1+x)^kappa - 1 = x (c0 + c1 x + ... + c11 x^11), kappa = Rd/cv
   double xmax;   // series used for |x| < xmax
 };
+
+// 1/a to within an ulp: hardware seed (relative error 2^-23) and two Newton steps; a is a density, never 0 / inf / nan
+__device__ __forceinline__ double rcp(double a) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+  double e = fma(-a, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-a, r, 1.0);
+  return fma(r, e, r);
+}
 
 template <int OVT>
 __device__ __forceinline__ double vflux(int ov, int r, double M, const double *w) {
@@ -72,11 +92,10 @@ __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 1, %0;\n" ::
 // the whole march of one thread; GRP (warp-uniform) selects the fields it advances, so that each role keeps only
 // its own vertical windows and FIFOs in registers
 template <int OH, int OVT, int GRP>
-__device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const int kchunk, double *sm) {
+__device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const Maps &maps, const int kchunk, double *sm) {
   double *const raw = sm;
   double *const prim = raw + NS * RAW;
-  double *const fifo = prim + NPB * PB;
-  uint64_t *const full = reinterpret_cast<uint64_t *>(fifo + NCOL * 4 * 2);
+  double *const tab = prim + NPB * PB;
 
   const int tid = threadIdx.x, t = tid & 255, tx = t & 31, ty = t >> 5;
   const int nx = p.nx, ny = p.ny, nz = p.nz, ov = p.ov;
@@ -88,6 +107,16 @@ __device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const
   const int Ls = max(k0 - 3, 0);                                  // first front level
   const int Ld = min(k1 + 2, nz);                                 // last level with data (nz: the W lid only)
   const int Lf = k1 + 2;                                          // last front level (flushes the FIFOs)
+  const int nlev = nz + 1;
+  uint64_t *const full = reinterpret_cast<uint64_t *>(tab + NTAB * nlev);
+  // per-level tables: shared memory instead of a dependent global load per level
+  const double *const t_dz = tab, *const t_rdz = tab + nlev, *const t_rhw = tab + 2 * nlev, *const t_rho0 = tab + 3 * nlev;
+  const double *const t_Th0 = tab + 4 * nlev, *const t_rTh0 = tab + 5 * nlev, *const t_p0 = tab + 6 * nlev,
+                      *const t_pi0 = tab + 7 * nlev;
+  for (int n = tid; n < nlev; n += NTH) {
+    tab[n] = p.dz[n]; tab[nlev + n] = p.rdz[n]; tab[2 * nlev + n] = p.rhw[n]; tab[3 * nlev + n] = p.rho0[n];
+    tab[4 * nlev + n] = p.Th0[n]; tab[5 * nlev + n] = p.rTh0[n]; tab[6 * nlev + n] = p.p0[n]; tab[7 * nlev + n] = p.pi0[n];
+  }
 
   if (GRP == 0 && tid == 0) {
 #pragma unroll
@@ -96,51 +125,76 @@ __device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const
   }
   cta_sync();
 
-  // ---- producer: one level = 72 row copies (rho: 16 rows, U, V, W, Theta: 14 rows), one per thread
-  const int gxs = pmodi(x0 - HX, nx);
-  int cp_f = -1, cp_row = 0, cp_gy = 0;
-  if (tid < NCOPY) {
-    if (tid < TH) { cp_f = 0; cp_row = tid; }
-    else { cp_f = 1 + (tid - TH) / (TH - 2); cp_row = 1 + (tid - TH) % (TH - 2); }
-    cp_gy = pmodi(y0 - HY + cp_row, ny);
+  // ---- producer: one level = 72 row copies (rho: 16 rows, U, V, W, Theta: 14 rows)
+  int cp_f = -1, cp_off = 0, cp_gy = 0;
+  const double *cp_src = nullptr;
+  // (the copies are spread over all 16 warps, five lanes each: a warp issues its bulk copies one lane at a time)
+  const int cpn = (tid & 31) < 5 ? (tid >> 5) * 5 + (tid & 31) : NCOPY;
+  if (cpn < NCOPY) {
+    int row;
+    if (cpn < TH) { cp_f = 0; row = cpn; }
+    else { cp_f = 1 + (cpn - TH) / (TH - 2); row = 1 + (cpn - TH) % (TH - 2); }
+    cp_gy = pmodi(y0 - HY + row, ny);
+    cp_off = cp_f * TSZ + row * TW;
+    cp_src = cp_f == 0 ? p.rho : cp_f == 1 ? p.U : cp_f == 2 ? p.V : cp_f == 3 ? p.W : p.Th;
   }
-  auto issue = [&](int lv) {
-    double *st = raw + (lv % NS) * RAW;
-    uint64_t *bar = &full[lv % NS];
-    if (tid == 0) mbar_arrive_expect_tx(bar, (unsigned)((lv < nz ? NCOPY : TH - 2) * TW * 8));
-    if (cp_f >= 0 && (lv < nz || cp_f == 3)) {
-      const double *src = cp_f == 0 ? p.rho : cp_f == 1 ? p.U : cp_f == 2 ? p.V : cp_f == 3 ? p.W : p.Th;
-      bulk_row(st + cp_f * TSZ + cp_row * TW, src + (size_t)lv * plane, cp_gy, gxs, TW, nx, bar);
+  const int gxs = pmodi(x0 - HX, nx);
+  // a CTA whose halo tile lies inside the domain gets each field plane with ONE tensor copy
+  const bool inside = p.use_tma && x0 >= HX && x0 + TX + HX <= nx && y0 >= HY && y0 + TY + HY <= ny;
+  auto issue = [&](int lv, int slot) {
+    uint64_t *bar = &full[slot];
+    if (inside) {
+      if (tid == 0) {
+        double *st = raw + slot * RAW;
+        if (lv < nz) {
+          mbar_arrive_expect_tx(bar, (unsigned)(5 * TSZ * 8));
+#pragma unroll
+          for (int f = 0; f < 5; f++) tma_tile_g2s(st + f * TSZ, &maps.m[f], x0 - HX, y0 - HY, lv, bar);
+        } else {
+          mbar_arrive_expect_tx(bar, (unsigned)(TSZ * 8));
+          tma_tile_g2s(st + 3 * TSZ, &maps.m[3], x0 - HX, y0 - HY, lv, bar);
+        }
+      }
+      return;
     }
+    if (tid == 0) mbar_arrive_expect_tx(bar, (unsigned)((lv < nz ? NCOPY : TH - 2) * TW * 8));
+    if (cp_f >= 0 && (lv < nz || cp_f == 3))
+      bulk_row(raw + slot * RAW + cp_off, cp_src + (size_t)lv * plane, cp_gy, gxs, TW, nx, bar);
   };
   unsigned phase = 0;
-  auto wait_level = [&](int lv) {
-    const int s = lv % NS;
+  auto wait_slot = [&](int s) {
     mbar_wait(&full[s], (phase >> s) & 1u);
     phase ^= 1u << s;
   };
 
-  // ---- primitives of level P into buffer P % NPB (every thread: one tile point)
-  const int ppt = tid, ppy = ppt / TW, ppx = ppt - ppy * TW;
-  const bool p_on = ppt < TSZ && ppy >= 1 && ppy <= TH - 2;
-  const bool p_pp = p_on && ppx >= 3 && ppx <= TX + HX - 1 && ppy >= 3 && ppy <= TY + HY - 1;    // p' region
+  // ---- primitives of level P (raw tile r, the level below in rm) into primitive buffer q.  The stencils never
+  // touch the corners of the halo, so the points needed form a cross: rows 4..11 x columns 1..38 and rows 1..3,
+  // 12..14 x columns 4..35 -- 496 points, one per thread in a single pass.
+  int ppx, ppy;
+  if (tid < 8 * 38) { ppy = HY + tid / 38; ppx = 1 + tid % 38; }
+  else { const int t2 = tid - 8 * 38, rr = t2 >> 5; ppy = rr < 3 ? 1 + rr : 9 + rr; ppx = HX + (t2 & 31); }
+  const bool p_on = tid < 8 * 38 + 6 * 32;
+  const int ppt = ppy * TW + ppx;
+  const bool p_pp = p_on && ppx >= 3 && ppx <= TX + HX - 1 && ppy >= 3 && ppy <= TY + HY - 1;  // p' region
   const int p_gi = x0 + ppx - HX, p_gj = y0 + ppy - HY;
-  const bool p_int = p_on && ppx >= HX && ppx < HX + TX && ppy >= HY && ppy < HY + TY && p_gi < nx && p_gj < ny;
-  auto prim_phase = [&](int P) {
+  const bool p_int = p_pp && ppx >= HX && ppy >= HY && p_gi < nx && p_gj < ny;
+  const size_t p_oc = p_int ? (size_t)p_gj * nx + p_gi : 0;
+  auto prim_phase = [&](int P, const double *__restrict__ r, const double *__restrict__ rm, double *__restrict__ q) {
     if (!p_on) return;
-    const double *__restrict__ r = raw + (P % NS) * RAW;
-    double *__restrict__ q = prim + (P % NPB) * PB;
     const double W = r[3 * TSZ + ppt];
     if (P < nz) {
       const double rc = r[ppt], Th = r[4 * TSZ + ppt];
-      q[ppt] = Th / rc;
-      if (ppx >= 1) q[TSZ + ppt] = r[TSZ + ppt] / (0.5 * (r[ppt - 1] + rc));
-      q[2 * TSZ + ppt] = r[2 * TSZ + ppt] / (0.5 * (r[ppt - TW] + rc));
-      const double rw = P == 0 ? rc : 0.5 * (raw[((P - 1) % NS) * RAW + ppt] + rc);
-      q[3 * TSZ + ppt] = W / rw;
+      const double th = Th * rcp(rc);
+      const double u = r[TSZ + ppt] * rcp(0.5 * (r[ppt - 1] + rc));
+      const double v = r[2 * TSZ + ppt] * rcp(0.5 * (r[ppt - TW] + rc));
+      const double w = W * rcp(P == 0 ? rc : 0.5 * (rm[ppt] + rc));
+      q[ppt] = th;
+      q[TSZ + ppt] = u;
+      q[2 * TSZ + ppt] = v;
+      q[3 * TSZ + ppt] = w;
       if (p_pp) {
         // x = Theta/Theta0 - 1, e = (1+x)^(Rd/cv) - 1: p' = p0 (x + e + x e), pi = pi0 (1 + e)   [R:S1]
-        const double x = (Th - p.Th0[P]) * p.rTh0[P];
+        const double x = (Th - t_Th0[P]) * t_rTh0[P];
         double e;
         if (fabs(x) < poly.xmax) {
           e = poly.c[11];
@@ -150,56 +204,66 @@ __device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const
         } else {
           e = expm1(p.rdocv * log1p(x));
         }
-        q[4 * TSZ + (ppy - 3) * PW + ppx - 2] = p.p0[P] * (x + e + x * e);
+        q[4 * TSZ + (ppy - 3) * PW + ppx - 2] = t_p0[P] * (x + e + x * e);
         if (p_int && P >= k0 && P < k1) {
-          const size_t a = (size_t)P * plane + (size_t)p_gj * nx + p_gi;
-          p.theta[a] = q[ppt];
-          p.pi[a] = p.pi0[P] * (1.0 + e);
-          p.iT[a] = 1.0 / Th;
+          const size_t a = (size_t)P * plane + p_oc;
+          p.theta[a] = th;
+          p.pi[a] = t_pi0[P] * (1.0 + e);
+          p.iT[a] = rcp(Th);
           if (p.diffusion != 0) {  // the diffusion kernels still read u, v, w from HBM
-            p.u[a] = q[TSZ + ppt];
-            p.v[a] = q[2 * TSZ + ppt];
-            p.w[a] = q[3 * TSZ + ppt];
+            p.u[a] = u;
+            p.v[a] = v;
+            p.w[a] = w;
           }
         }
       }
     } else {
-      const double wl = W / raw[((P - 1) % NS) * RAW + ppt];  // face nz: rho_w = rho(nz-1)
-      q[3 * TSZ + ppt] = wl;
-      if (p_int && k1 == nz && p.diffusion != 0) p.w[(size_t)P * plane + (size_t)p_gj * nx + p_gi] = wl;
+      const double w = W * rcp(rm[ppt]);  // face nz: rho_w = rho(nz-1)
+      q[3 * TSZ + ppt] = w;
+      if (p_int && k1 == nz && p.diffusion != 0) p.w[(size_t)P * plane + p_oc] = w;
     }
   };
 
-  // ---- prologue: levels Ls-1 (for rho below the first face), Ls, Ls+1
-  for (int lv = max(Ls - 1, 0); lv <= min(Ls + 1, Ld); lv++) issue(lv);
-  if (Ls >= 1) wait_level(Ls - 1);
+  // ---- prologue: levels Ls-1 (for rho below the first face) .. Ls+2
+  int sP = Ls % NS;  // raw slot of level P
+  {
+    const int lo = max(Ls - 1, 0);
+    for (int lv = lo; lv <= min(Ls + 2, Ld); lv++) issue(lv, lv % NS);
+    if (Ls >= 1) wait_slot((Ls - 1) % NS);
+  }
+  int bP = Ls % NPB;  // primitive buffer of level P
+  cta_sync();         // the tables
 
   const double rdx = p.rdx, rdy = p.rdy;
   const size_t oc = act ? (size_t)j * nx + i : 0;
   const int c = (ty + HY) * TW + tx + HX;           // own column in a TW x TH tile
   const int cP = (ty + 1) * PW + tx + 2;            // own column in the p' tile
-  double *const myfifo = fifo + t;                  // group 1: [(slot * 2 + f) * NCOL]
 
-  // per-thread state (each group uses its own subset; the compiler drops the rest per branch)
-  double win[6] = {0, 0, 0, 0, 0, 0}, win2[6] = {0, 0, 0, 0, 0, 0};  // vertical windows
-  double omw[4] = {0, 0, 0, 0};                                      // Omega at faces L-3 .. L (own column / averaged)
-  double omv[3] = {0, 0, 0};                                         // group 1: Mz for v at faces L-2 .. L
-  double f0[3] = {0, 0, 0}, f1[3] = {0, 0, 0};                       // parked horizontal parts of cells L-3 .. L-1
-  double fb0 = 0.0, fb1 = 0.0;                                       // vertical flux at the bottom face of the cell being finished
-  double U_cm = 0.0, U_pm = 0.0, V_cm = 0.0, V_pm = 0.0, pp_m = 0.0, rp_m = 0.0;  // group 2: level L-1
+  // per-thread state
+  double win[6] = {0, 0, 0, 0, 0, 0}, win2[6] = {0, 0, 0, 0, 0, 0};  // vertical windows: (theta, w) or (u, v)
+  double omw[4] = {0, 0, 0, 0};                                      // Omega at faces L-3 .. L (group 1: averaged to the u-point)
+  double omv[3] = {0, 0, 0};                                         // group 1: Omega averaged to the v-point, faces L-2 .. L
+  double f0[3] = {0, 0, 0}, f1[3] = {0, 0, 0}, f2[3] = {0, 0, 0};    // parked horizontal parts of levels L-3 .. L-1
+  double fb0 = 0.0, fb1 = 0.0;                                       // vertical fluxes carried from the face below
+  double U_cm = 0.0, U_pm = 0.0, V_cm = 0.0, V_pm = 0.0, pp_m = 0.0, rp_m = 0.0;  // group 0, rho*w: level L-1
 
+  // One iteration: primitives of the level that has just landed (P), then the column work two levels below
+  // (front level L = P-2, whose primitives were finished two iterations ago), ONE barrier, then the refill of the
+  // raw slot that the front level has just released.  The two halves of an iteration touch different buffers, so
+  // they overlap freely within and across warps.
 #pragma unroll 1
-  for (int P = Ls; P <= Lf + 1; P++) {
+  for (int P = Ls; P <= Lf + 2; P++) {
+    const int sM = sP == 0 ? NS - 1 : sP - 1;        // raw slot of level P-1
+    const int sL = sM == 0 ? NS - 1 : sM - 1;        // raw slot of level P-2 (= the front level L)
+    const int bL = bP == NPB - 1 ? 0 : bP + 1;       // (P-2) % 3 == (P+1) % 3
     if (P <= Ld) {
-      wait_level(P);
-      prim_phase(P);
+      wait_slot(sP);
+      prim_phase(P, raw + sP * RAW, raw + sM * RAW, prim + bP * PB);
     }
-    cta_sync();
-    if (P + 2 <= Ld) issue(P + 2);
-    const int L = P - 1;
-    if (L < Ls || !act) continue;
-    const double *__restrict__ r = raw + (L % NS) * RAW;
-    const double *__restrict__ q = prim + (L % NPB) * PB;
+    const int L = P - 2;
+    if (L >= Ls && act) {
+    const double *__restrict__ r = raw + sL * RAW;
+    const double *__restrict__ q = prim + bL * PB;
     const double *__restrict__ mU = r + TSZ, *__restrict__ mV = r + 2 * TSZ, *__restrict__ mW = r + 3 * TSZ;
     const bool cell = L < nz;                        // a cell level with data
     const bool inner = L >= 1 && L <= nz - 1;        // an interior w-face
@@ -207,44 +271,62 @@ __device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const
     const bool fin = kc >= k0 && kc < k1;
 
     if (GRP == 0) {
-      // ------------------------------------------------ rho, rho*theta
-      double Hr = 0.0, HT = 0.0, th = 0.0;
+      // ------------------------------------------------ rho, rho*theta; rho*w at face L with PG_z and buoyancy
+      const double *__restrict__ sW = q + 3 * TSZ, *__restrict__ sPp = q + 4 * TSZ;
+      double Hr = 0.0, HT = 0.0, X = 0.0, th = 0.0, wc = 0.0;
+      if (L <= nz) wc = sW[c];
       if (cell) {
         const double U_c = mU[c], U_p = mU[c + 1], V_c = mV[c], V_p = mV[c + TW];
         Hr = (U_p - U_c) * rdx + (V_p - V_c) * rdy;
         HT = hdiv_x<OH>(q, c, U_c, U_p) * rdx + hdiv_y<OH>(q, c, V_c, V_p) * rdy;
         th = q[c];
+        const double dzk = t_dz[L];
+        const double U_cd = dzk * U_c, U_pd = dzk * U_p, V_cd = dzk * V_c, V_pd = dzk * V_p;
+        const double pp_c = sPp[cP], rp_c = r[c] - t_rho0[L];
+        if (L >= 1) {
+          const double rhw = t_rhw[L];
+          const double adv = hdiv_x<OH>(sW, c, 0.5 * (U_cm + U_cd), 0.5 * (U_pm + U_pd)) * rdx +
+                             hdiv_y<OH>(sW, c, 0.5 * (V_cm + V_cd), 0.5 * (V_pm + V_pd)) * rdy;
+          X = -adv * rhw - ((pp_c - pp_m) * rhw + p.g * 0.5 * (rp_m + rp_c));
+        }
+        U_cm = U_cd; U_pm = U_pd; V_cm = V_cd; V_pm = V_pd;
+        pp_m = pp_c; rp_m = rp_c;
       }
 #pragma unroll
-      for (int n = 0; n < 5; n++) win[n] = win[n + 1];
-      win[5] = th;
+      for (int n = 0; n < 5; n++) { win[n] = win[n + 1]; win2[n] = win2[n + 1]; }
+      win[5] = th;                                   // cells L-5 .. L
+      win2[5] = wc;                                  // faces L-5 .. L
       omw[0] = omw[1]; omw[1] = omw[2]; omw[2] = omw[3];
       omw[3] = inner ? mW[c] : 0.0;                  // Omega = W on a flat grid; 0 on the lids
-      double fT = 0.0;
+      double fT = 0.0, Gz = 0.0;
       if (kf >= 1 && kf <= nz - 1) fT = vflux<OVT>(ov, min(kf, nz - kf), omw[1], win);
+      // vertical flux of w at centre kc (between faces kc and kc+1)
+      if (kc >= 0 && kc <= nz - 1) Gz = vflux<OVT>(ov, min(kc + 1, nz - kc), 0.5 * (omw[0] + omw[1]), win2);
       if (fin) {
-        const double rdzc = p.rdz[kc];
+        const double rdzc = t_rdz[kc];
         const size_t a = (size_t)kc * plane + oc;
         p.Rrho[a] = -(f0[0] + (omw[1] - omw[0]) * rdzc);
         p.RTh[a] = -(f1[0] + (fT - fb0) * rdzc);
+        p.RW[a] = kc >= 1 ? f2[0] - (Gz - fb1) * t_rhw[kc] : 0.0;
+        if (kc == nz - 1) p.RW[a + plane] = 0.0;     // upper lid
       }
       fb0 = fT;
+      fb1 = Gz;
       f0[0] = f0[1]; f0[1] = f0[2]; f0[2] = Hr;
       f1[0] = f1[1]; f1[1] = f1[2]; f1[2] = HT;
-    } else if (GRP == 1) {
+      f2[0] = f2[1]; f2[1] = f2[2]; f2[2] = X;
+    } else {
       // ------------------------------------------------ rho*u, rho*v
-      const double *__restrict__ sU = q + TSZ, *__restrict__ sV = q + 2 * TSZ, *__restrict__ sP = q + 4 * TSZ;
-      double uc = 0.0, vc = 0.0;
+      const double *__restrict__ sU = q + TSZ, *__restrict__ sV = q + 2 * TSZ, *__restrict__ sPp = q + 4 * TSZ;
+      double HU = 0.0, HV = 0.0, uc = 0.0, vc = 0.0;
       if (cell) {
         const double U_m = mU[c - 1], U_c = mU[c], U_p = mU[c + 1], U_ym = mU[c - TW], U_pym = mU[c - TW + 1];
         const double V_m = mV[c - TW], V_c = mV[c], V_p = mV[c + TW], V_xm = mV[c - 1], V_xmp = mV[c + TW - 1];
-        const double pp_c = sP[cP];
-        const double HU = hdiv_x<OH>(sU, c, 0.5 * (U_m + U_c), 0.5 * (U_c + U_p)) * rdx +
-                          hdiv_y<OH>(sU, c, 0.5 * (V_xm + V_c), 0.5 * (V_xmp + V_p)) * rdy + (pp_c - sP[cP - 1]) * rdx;
-        const double HV = hdiv_x<OH>(sV, c, 0.5 * (U_ym + U_c), 0.5 * (U_pym + U_p)) * rdx +
-                          hdiv_y<OH>(sV, c, 0.5 * (V_m + V_c), 0.5 * (V_c + V_p)) * rdy + (pp_c - sP[cP - PW]) * rdy;
-        myfifo[((L & 3) * 2) * NCOL] = HU;
-        myfifo[((L & 3) * 2 + 1) * NCOL] = HV;
+        const double pp_c = sPp[cP];
+        HU = hdiv_x<OH>(sU, c, 0.5 * (U_m + U_c), 0.5 * (U_c + U_p)) * rdx +
+             hdiv_y<OH>(sU, c, 0.5 * (V_xm + V_c), 0.5 * (V_xmp + V_p)) * rdy + (pp_c - sPp[cP - 1]) * rdx;
+        HV = hdiv_x<OH>(sV, c, 0.5 * (U_ym + U_c), 0.5 * (U_pym + U_p)) * rdx +
+             hdiv_y<OH>(sV, c, 0.5 * (V_m + V_c), 0.5 * (V_c + V_p)) * rdy + (pp_c - sPp[cP - PW]) * rdy;
         uc = sU[c];
         vc = sV[c];
       }
@@ -268,57 +350,30 @@ __device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const
         fV = vflux<OVT>(ov, rr, omv[0], win2);
       }
       if (fin) {
-        const double rdzc = p.rdz[kc];
+        const double rdzc = t_rdz[kc];
         const size_t a = (size_t)kc * plane + oc;
-        p.RU[a] = -(myfifo[((kc & 3) * 2) * NCOL] + (fU - fb0) * rdzc);
-        p.RV[a] = -(myfifo[((kc & 3) * 2 + 1) * NCOL] + (fV - fb1) * rdzc);
+        p.RU[a] = -(f0[0] + (fU - fb0) * rdzc);
+        p.RV[a] = -(f1[0] + (fV - fb1) * rdzc);
       }
       fb0 = fU;
       fb1 = fV;
-    } else {
-      // ------------------------------------------------ rho*w at face L, pressure gradient and buoyancy
-      const double *__restrict__ sW = q + 3 * TSZ, *__restrict__ sP = q + 4 * TSZ;
-      double X = 0.0, wc = 0.0;
-      if (L <= nz) wc = sW[c];
-      if (cell) {
-        const double dzk = p.dz[L];
-        const double U_cd = dzk * mU[c], U_pd = dzk * mU[c + 1], V_cd = dzk * mV[c], V_pd = dzk * mV[c + TW];
-        const double pp_c = sP[cP], rp_c = r[c] - p.rho0[L];
-        if (L >= 1) {
-          const double rhw = p.rhw[L];
-          const double adv = hdiv_x<OH>(sW, c, 0.5 * (U_cm + U_cd), 0.5 * (U_pm + U_pd)) * rdx +
-                             hdiv_y<OH>(sW, c, 0.5 * (V_cm + V_cd), 0.5 * (V_pm + V_pd)) * rdy;
-          X = -adv * rhw - ((pp_c - pp_m) * rhw + p.g * 0.5 * (rp_m + rp_c));
-        }
-        U_cm = U_cd; U_pm = U_pd; V_cm = V_cd; V_pm = V_pd;
-        pp_m = pp_c; rp_m = rp_c;
-      }
-#pragma unroll
-      for (int n = 0; n < 5; n++) win[n] = win[n + 1];
-      win[5] = wc;                                   // faces L-5 .. L
-      omw[0] = omw[1]; omw[1] = omw[2]; omw[2] = omw[3];
-      omw[3] = inner ? mW[c] : 0.0;
-      // vertical flux of w at centre kc (between faces kc and kc+1)
-      double Gz = 0.0;
-      if (kc >= 0 && kc <= nz - 1) Gz = vflux<OVT>(ov, min(kc + 1, nz - kc), 0.5 * (omw[0] + omw[1]), win);
-      if (fin) {
-        const size_t a = (size_t)kc * plane + oc;
-        p.RW[a] = kc >= 1 ? f0[0] - (Gz - fb0) * p.rhw[kc] : 0.0;
-        if (kc == nz - 1) p.RW[a + plane] = 0.0;     // upper lid
-      }
-      fb0 = Gz;
-      f0[0] = f0[1]; f0[1] = f0[2]; f0[2] = X;
+      f0[0] = f0[1]; f0[1] = f0[2]; f0[2] = HU;
+      f1[0] = f1[1]; f1[1] = f1[2]; f1[2] = HV;
     }
+    }
+    cta_sync();
+    if (P + 3 <= Ld) issue(P + 3, sL);               // level P+3 takes the slot of level P-2
+    sP = sP == NS - 1 ? 0 : sP + 1;
+    bP = bL;
   }
 }
 
 template <int OH, int OVT>
-__global__ void __launch_bounds__(NTH, 1) k_slow_adv(const SlowFlat p, const Poly poly, const int kchunk) {
+__global__ void __launch_bounds__(NTH, 1)
+    k_slow_adv(const SlowFlat p, const Poly poly, const __grid_constant__ Maps maps, const int kchunk) {
   extern __shared__ __align__(128) double sm[];
-  const int grp = threadIdx.x >> 8;
-  if (grp == 0) march<OH, OVT, 0>(p, poly, kchunk, sm);
-  else if (grp == 1) march<OH, OVT, 1>(p, poly, kchunk, sm);
-  else march<OH, OVT, 2>(p, poly, kchunk, sm);
+  if (threadIdx.x < NCOL) march<OH, OVT, 0>(p, poly, maps, kchunk, sm);
+  else march<OH, OVT, 1>(p, poly, maps, kchunk, sm);
 }
 
 }  // namespace sadv
@@ -335,19 +390,21 @@ static sadv::Poly make_poly(double kappa) {
   return P;
 }
 
-bool slow_adv_available(const erf_ctx *c) { return (c->nx % 2) == 0; }
+bool slow_adv_available(const erf_ctx *c) { return (c->nx % 2) == 0 && c->nz + 1 <= sadv::MAXLEV; }
 
 template <int OH, int OVT>
-static void launch_one(const SlowFlat &p, const sadv::Poly &poly, dim3 grid, int kchunk, cudaStream_t st) {
+static void launch_one(const SlowFlat &p, const sadv::Poly &poly, const sadv::Maps &maps, dim3 grid, int kchunk,
+                       cudaStream_t st) {
   static bool once = false;
   if (!once) {
-    cudaFuncSetAttribute(sadv::k_slow_adv<OH, OVT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sadv::SMEM);
+    cudaFuncSetAttribute(sadv::k_slow_adv<OH, OVT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                         (int)sadv::smem_bytes(sadv::MAXLEV));
     once = true;
   }
-  sadv::k_slow_adv<OH, OVT><<<grid, sadv::NTH, sadv::SMEM, st>>>(p, poly, kchunk);
+  sadv::k_slow_adv<OH, OVT><<<grid, sadv::NTH, sadv::smem_bytes(p.nz + 1), st>>>(p, poly, maps, kchunk);
 }
 
-void launch_slow_adv(erf_ctx *c, const SlowFlat &p, cudaStream_t st) {
+void launch_slow_adv(erf_ctx *c, const SlowFlat &pin, cudaStream_t st) {
   using namespace sadv;
   const int gx = (c->nx + TX - 1) / TX, gy = (c->ny + TY - 1) / TY;
   // level chunks so that a small grid still gives every SM a CTA (each chunk recomputes 6 levels)
@@ -357,13 +414,28 @@ void launch_slow_adv(erf_ctx *c, const SlowFlat &p, cudaStream_t st) {
   const int kchunk = (c->nz + nch - 1) / nch;
   dim3 grid(gx, gy, (c->nz + kchunk - 1) / kchunk);
   const Poly poly = make_poly(c->v.rdocv);
+  // tensor maps of the five input fields (cached per buffer: the state buffers rotate between steps)
+  SlowFlat p = pin;
+  Maps maps;
+  memset(&maps, 0, sizeof(maps));
+  p.use_tma = 1;
+  const double *src[5] = {p.rho, p.U, p.V, p.W, p.Th};
+  for (int f = 0; f < 5 && p.use_tma; f++) {
+    auto it = c->fz->tmaps.find(src[f]);
+    if (it == c->fz->tmaps.end()) {
+      CUtensorMap m;
+      if (!make_tile_map(&m, src[f], c->nx, c->ny, c->nz + 1, sadv::TW, sadv::TH)) { p.use_tma = 0; break; }
+      it = c->fz->tmaps.emplace(src[f], m).first;
+    }
+    maps.m[f] = it->second;
+  }
   const bool same = c->p.adv_order_h == c->p.adv_order_v;
   switch (c->p.adv_order_h) {
-    case 2: same ? launch_one<2, 2>(p, poly, grid, kchunk, st) : launch_one<2, 0>(p, poly, grid, kchunk, st); break;
-    case 3: same ? launch_one<3, 3>(p, poly, grid, kchunk, st) : launch_one<3, 0>(p, poly, grid, kchunk, st); break;
-    case 4: same ? launch_one<4, 4>(p, poly, grid, kchunk, st) : launch_one<4, 0>(p, poly, grid, kchunk, st); break;
-    case 5: same ? launch_one<5, 5>(p, poly, grid, kchunk, st) : launch_one<5, 0>(p, poly, grid, kchunk, st); break;
-    default: same ? launch_one<6, 6>(p, poly, grid, kchunk, st) : launch_one<6, 0>(p, poly, grid, kchunk, st); break;
+    case 2: same ? launch_one<2, 2>(p, poly, maps, grid, kchunk, st) : launch_one<2, 0>(p, poly, maps, grid, kchunk, st); break;
+    case 3: same ? launch_one<3, 3>(p, poly, maps, grid, kchunk, st) : launch_one<3, 0>(p, poly, maps, grid, kchunk, st); break;
+    case 4: same ? launch_one<4, 4>(p, poly, maps, grid, kchunk, st) : launch_one<4, 0>(p, poly, maps, grid, kchunk, st); break;
+    case 5: same ? launch_one<5, 5>(p, poly, maps, grid, kchunk, st) : launch_one<5, 0>(p, poly, maps, grid, kchunk, st); break;
+    default: same ? launch_one<6, 6>(p, poly, maps, grid, kchunk, st) : launch_one<6, 0>(p, poly, maps, grid, kchunk, st); break;
   }
   c->launches++;
 }

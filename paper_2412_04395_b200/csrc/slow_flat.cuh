@@ -14,6 +14,7 @@ struct SlowFlat {
   const double *dz, *rdz, *rhw, *rho0, *Th0, *rTh0, *p0, *pi0, *csd2;
   double gam, rdocv, nu, alpha, rPrt;
   int diffusion;
+  int use_tma;  // k_slow_adv: tensor maps are valid
 };
 
 // ------------------------------------------------------------------ Eq. 17-21
