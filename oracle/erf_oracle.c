@@ -75,6 +75,7 @@ static int wrapi(int a, int n) {
 
 /* periodic lateral boundary: ghost = image of the interior */
 static void fill_periodic(const erfo_ctx *c, double *f) {
+#pragma omp parallel for schedule(static)
   for (int k = 0; k <= c->nz; k++)
     for (int j = -NG; j < c->ny + NG; j++)
       for (int i = -NG; i < c->nx + NG; i++)
@@ -83,6 +84,7 @@ static void fill_periodic(const erfo_ctx *c, double *f) {
 }
 
 static void put_dense(const erfo_ctx *c, double *f, const double *dense, int nlev) {
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nlev; k++)
     for (int j = 0; j < c->ny; j++)
       for (int i = 0; i < c->nx; i++)
@@ -91,6 +93,7 @@ static void put_dense(const erfo_ctx *c, double *f, const double *dense, int nle
 }
 
 static void get_dense(const erfo_ctx *c, const double *f, double *dense, int nlev) {
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nlev; k++)
     for (int j = 0; j < c->ny; j++)
       for (int i = 0; i < c->nx; i++)
@@ -185,6 +188,7 @@ void erfo_eos(double Rd, double cp, double p00, double Theta, double Theta0, dou
 static void build_geometry(erfo_ctx *c, const double *zn) {
   int nx = c->nx, ny = c->ny, nz = c->nz;
 #define ZN(i, j, k) zn[((size_t)(k) * (ny + 1) + (j)) * (nx + 1) + (i)]
+#pragma omp parallel for schedule(static)
   for (int k = 0; k <= nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -197,6 +201,7 @@ static void build_geometry(erfo_ctx *c, const double *zn) {
   fill_periodic(c, c->zxf);
   fill_periodic(c, c->zyf);
   fill_periodic(c, c->zw);
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -209,11 +214,13 @@ static void build_geometry(erfo_ctx *c, const double *zn) {
   fill_periodic(c, c->hy);
   fill_periodic(c, c->hc);
   fill_periodic(c, c->zc);
+#pragma omp parallel for schedule(static)
   for (int k = 1; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++)
         c->hw[IX(c, i, j, k)] = c->zc[IX(c, i, j, k)] - c->zc[IX(c, i, j, k - 1)];
   fill_periodic(c, c->hw);
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -226,6 +233,7 @@ static void build_geometry(erfo_ctx *c, const double *zn) {
   fill_periodic(c, c->hv);
   fill_periodic(c, c->sxu);
   fill_periodic(c, c->syv);
+#pragma omp parallel for schedule(static)
   for (int k = 0; k <= nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -263,6 +271,7 @@ static void impose_lids(const erfo_ctx *c, const double *U, const double *V, dou
 static void contravariant_flux(const erfo_ctx *c, const double *U, const double *V,
                                const double *W, double *Om) {
   int nz = c->nz;
+#pragma omp parallel for schedule(static)
   for (int k = 0; k <= nz; k++)
     for (int j = 0; j < c->ny; j++)
       for (int i = 0; i < c->nx; i++) {
@@ -293,6 +302,7 @@ typedef struct {
  * adjacent cells [R:G11]; at the lids rho_w = adjacent cell. */
 static void primitives(const erfo_ctx *c, double *const S[5], prim_t *q) {
   int nx = c->nx, ny = c->ny, nz = c->nz;
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -303,6 +313,7 @@ static void primitives(const erfo_ctx *c, double *const S[5], prim_t *q) {
         q->u[a] = S[UU][a] / (0.5 * (S[RHO][IX(c, i - 1, j, k)] + S[RHO][a]));
         q->v[a] = S[VV][a] / (0.5 * (S[RHO][IX(c, i, j - 1, k)] + S[RHO][a]));
       }
+#pragma omp parallel for schedule(static)
   for (int k = 0; k <= nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -332,6 +343,7 @@ static void advection(const erfo_ctx *c, double *const S[5], const prim_t *q, do
   /* mass fluxes through cell faces: Fx = hx U, Fy = hy V (face-height
    * weighted, finite-volume form [R:G14]) and Omega */
   double *Fx = fnew(c), *Fy = fnew(c), *Om = fnew(c);
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -343,6 +355,7 @@ static void advection(const erfo_ctx *c, double *const S[5], const prim_t *q, do
   fill_periodic(c, Fy);
   contravariant_flux(c, S[UU], S[VV], S[WW], Om);
 
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -401,6 +414,7 @@ static void advection(const erfo_ctx *c, double *const S[5], const prim_t *q, do
         }
       }
   /* ---- W momentum on interior faces k = 1..nz-1; R_W = 0 on the lids ---- */
+#pragma omp parallel for schedule(static)
   for (int k = 0; k <= nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -466,6 +480,7 @@ static void strain_and_viscosity(const erfo_ctx *c, double *const S[5], const pr
   int nx = c->nx, ny = c->ny, nz = c->nz;
   double dx = c->dx, dy = c->dy;
   /* vertical quotients of u and v at (i-1/2,j,k-1/2), (i,j-1/2,k-1/2); 0 on lids */
+#pragma omp parallel for schedule(static)
   for (int k = 1; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -478,6 +493,7 @@ static void strain_and_viscosity(const erfo_ctx *c, double *const S[5], const pr
   fill_periodic(c, d->qu);
   fill_periodic(c, d->qv);
   /* S33 first: it is also the vertical quotient of w at centres */
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -485,6 +501,7 @@ static void strain_and_viscosity(const erfo_ctx *c, double *const S[5], const pr
         d->S33[a] = (q->w[IX(c, i, j, k + 1)] - q->w[a]) / c->hc[a];
       }
   fill_periodic(c, d->S33);
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -520,6 +537,7 @@ static void strain_and_viscosity(const erfo_ctx *c, double *const S[5], const pr
 #undef ZCV
       }
   /* S13 at (i-1/2, j, k-1/2), S23 at (i, j-1/2, k-1/2); zero on the lids */
+#pragma omp parallel for schedule(static)
   for (int k = 1; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -545,6 +563,7 @@ static void strain_and_viscosity(const erfo_ctx *c, double *const S[5], const pr
   fill_periodic(c, d->S13);
   fill_periodic(c, d->S23);
   /* viscosity mu = mu_m + mu_t (L100) and scalar diffusivity K = rho*alpha */
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -589,6 +608,7 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
    * viscosity = 4-point mean of the centre values [R:G11]. */
   double *t11 = fnew(c), *t22 = fnew(c), *t33 = fnew(c);
   double *t12 = fnew(c), *t13 = fnew(c), *t23 = fnew(c);
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -616,12 +636,14 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
   double *q11 = fnew(c), *q22 = fnew(c), *q12 = fnew(c), *q13 = fnew(c), *q23 = fnew(c);
   double *qth = fnew(c);
   double *ze12 = fnew(c); /* height of the xy-edge: mean of the 4 cell centres */
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++)
         ze12[IX(c, i, j, k)] = 0.25 * (c->zc[IX(c, i - 1, j - 1, k)] + c->zc[IX(c, i, j - 1, k)] +
                                        c->zc[IX(c, i - 1, j, k)] + c->zc[IX(c, i, j, k)]);
   fill_periodic(c, ze12);
+#pragma omp parallel for schedule(static)
   for (int k = 1; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -632,6 +654,7 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
         q12[a] = (t12[a] - t12[b]) / (ze12[a] - ze12[b]);
       }
   /* tau13, tau23 live on k-1/2 edges; their quotients live at level centres 0..nz-1 */
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -647,6 +670,7 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
   fill_periodic(c, q13); fill_periodic(c, q23); fill_periodic(c, qth);
 
   /* ---- momentum: R -= div tau (non-conservative chain-rule form over terrain) ---- */
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -692,6 +716,7 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
    * contravariant Fzeta = Fz - sxw avg4(Fx) - syw avg4(Fy), zero on the lids.
    * Diffusion acts on the full theta (Eq. 3) [R:G17]. */
   double *Fx = fnew(c), *Fy = fnew(c), *Fz = fnew(c);
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -708,6 +733,7 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
       }
   fill_periodic(c, Fx);
   fill_periodic(c, Fy);
+#pragma omp parallel for schedule(static)
   for (int k = 1; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -720,6 +746,7 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
                              Fy[IX(c, i, j + 1, k)]);
         Fz[a] = fz - c->sxw[a] * fxb - c->syw[a] * fyb;
       } /* Fz = 0 on k = 0 and k = nz */
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -765,6 +792,7 @@ static double grad_y(const erfo_ctx *c, const double *f, int i, int j, int k) {
 static void pressure_buoyancy(const erfo_ctx *c, double *const S[5], const prim_t *q,
                               double *R[5]) {
   int nx = c->nx, ny = c->ny, nz = c->nz;
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -848,6 +876,7 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
 
   /* 1. divergence damping (L144): Theta'' "predicted slightly forward in time" [R:G6] */
   double *Thd = fnew(c);
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -858,6 +887,7 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
   fill_periodic(c, Thd);
 
   /* 2. horizontal momenta, explicit (L585 rows 1-2); pi^t averaged to the face */
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -872,6 +902,7 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
 
   /* 3. explicit slope part of W'': omega = sxw avg4(U''new) + syw avg4(V''new) [R:G16] */
   double *om = fnew(c);
+#pragma omp parallel for schedule(static)
   for (int k = 1; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {
@@ -881,7 +912,9 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
         om[a] = c->sxw[a] * ubar + c->syw[a] * vbar;
       }
 
-  /* 4.-6. per column */
+  /* 4.-6. per column (columns are independent: each thread of the optional OpenMP build owns its scratch) */
+#pragma omp parallel
+  {
   double *Ttil = (double *)calloc(nz, sizeof(double)), *rtil = (double *)calloc(nz, sizeof(double));
   double *That = (double *)calloc(nz, sizeof(double)), *rhat = (double *)calloc(nz, sizeof(double));
   double *thf = (double *)calloc(nz + 1, sizeof(double));
@@ -889,6 +922,7 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
   double *C = (double *)calloc(nz + 1, sizeof(double)), *rhs = (double *)calloc(nz + 1, sizeof(double));
   double *On = (double *)calloc(nz + 1, sizeof(double));
   double *cp_ = (double *)calloc(nz + 1, sizeof(double)), *dp_ = (double *)calloc(nz + 1, sizeof(double));
+#pragma omp for schedule(static)
   for (int j = 0; j < ny; j++)
     for (int i = 0; i < nx; i++) {
       /* theta^t at the w-faces; the lid values are never used (Omega = 0 there) */
@@ -952,6 +986,7 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
     }
   free(Ttil); free(rtil); free(That); free(rhat); free(thf);
   free(A); free(D); free(C); free(rhs); free(On); free(cp_); free(dp_);
+  }
   free(om);
   free(Thd);
   fill_periodic(c, Wpp);
@@ -1056,6 +1091,7 @@ int erfo_create(const erfo_grid *g, const erfo_metrics *m, const erfo_params *p,
   build_geometry(c, zn);
   free(zn);
   /* base state: rho0, Theta0 given; p0, pi0 from Eq. 7 [R:S1] */
+#pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++) {

@@ -40,15 +40,30 @@ class Params(C.Structure):
                 ("substep_mode", C.c_int)]
 
 
-def build(force: bool = False) -> str:
-    """Compile the oracle (plain C, no FMA contraction) if stale."""
-    if (not force and os.path.exists(_SO)
-            and os.path.getmtime(_SO) >= max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))):
-        return _SO
-    cmd = ["gcc", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=c99", "-Wall",
-           "-o", _SO, _SRC, "-lm"]
-    subprocess.check_call(cmd)
-    return _SO
+_SO_OMP = os.path.join(_HERE, "liberf_oracle_omp.so")
+_use_omp = False
+
+
+def build(force: bool = False, omp: bool = False) -> str:
+    """Compile the oracle (plain C, no FMA contraction) if stale.  ``omp``: the same source with -fopenmp
+    (bitwise-identical results, see erf_oracle.c; for the long parity runs only)."""
+    so = _SO_OMP if omp else _SO
+    if (not force and os.path.exists(so)
+            and os.path.getmtime(so) >= max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))):
+        return so
+    cmd = ["gcc", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-std=c99", "-Wall", "-Wno-unknown-pragmas"]
+    if omp:
+        cmd.append("-fopenmp")
+    subprocess.check_call(cmd + ["-o", so, _SRC, "-lm"])
+    return so
+
+
+def use_openmp(on: bool):
+    """Switch every Oracle created from now on to the OpenMP build (False: back to the serial build)."""
+    global _lib, _use_omp
+    if on != _use_omp:
+        _use_omp = on
+        _lib = None
 
 
 _lib = None
@@ -57,8 +72,7 @@ _lib = None
 def lib():
     global _lib
     if _lib is None:
-        build()
-        L = C.CDLL(_SO)
+        L = C.CDLL(build(omp=_use_omp))
         L.erfo_create.argtypes = [C.POINTER(Grid), C.POINTER(Metrics), C.POINTER(Params),
                                   C.POINTER(C.c_void_p)]
         L.erfo_set_state.argtypes = [C.c_void_p] + [_dp] * 5

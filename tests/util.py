@@ -45,3 +45,22 @@ def field_errors(got, ref):
     sm = max(max(float(np.abs(ref[f]).max()) for f in (1, 2, 3)), tiny)
     scale = [max(float(np.abs(ref[0]).max()), tiny), sm, sm, sm, max(float(np.abs(ref[4]).max()), tiny)]
     return [float(np.abs(got[f] - ref[f]).max() / scale[f]) for f in range(5)]
+
+
+def perturbation_errors(got, ref, case):
+    """A stricter companion of G24 (reported beside it): the error of each field relative to what
+    actually moves -- rho - rho0 and Theta - Theta0 against the largest perturbation, W against max|W| alone (not
+    the shared momentum scale), U and V against their largest departure from the horizontal mean of each level.
+    Order (rho', U', V', W, Theta')."""
+    got = [np.asarray(a) for a in got]
+    ref = [np.asarray(a) for a in ref]
+    r0, t0 = base_state_fields(case)
+    tiny = 1e-300
+
+    def dev(a):
+        return a - a.mean(axis=(1, 2), keepdims=True)
+
+    scale = [max(float(np.abs(ref[0] - r0).max()), tiny), max(float(np.abs(dev(ref[1])).max()), tiny),
+             max(float(np.abs(dev(ref[2])).max()), tiny), max(float(np.abs(ref[3]).max()), tiny),
+             max(float(np.abs(ref[4] - t0).max()), tiny)]
+    return [float(np.abs(got[f] - ref[f]).max() / scale[f]) for f in range(5)]
