@@ -50,12 +50,12 @@ def measured_peak_gbs():
 
 def measured_traffic(kernel_class, config):
     """DRAM bytes per launch of a kernel class from the committed ncu capture of config 5
-    (profiles/r1_dram_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum); None for other workloads."""
+    (profiles/r2_dram_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum); None for other workloads."""
     if config != 5:
         return None
     import csv
     try:
-        with open(os.path.join(ROOT, "profiles", "r1_dram_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")) as f:
             for row in csv.DictReader(f):
                 if row["kernel_class"] == kernel_class:
                     return float(row["bytes_per_launch"])
@@ -166,7 +166,11 @@ def run_reference(args):
     kw = sample_kw(args.config)
     value, spp, sample = time_oracle(kw, args.config, args.steps, args.warmup)
     case = wl.make_case(args.config, with_state=False, **kw)
-    cfg = config_desc(dict(case, nx=wl.CONFIGS[args.config]["nx"], ny=wl.CONFIGS[args.config]["ny"]), args.config)
+    cfg = config_desc(case, args.config)   # the crop's own nx, ny and cell count
+    full = wl.CONFIGS[args.config]
+    cfg["workload"] = (f"{case['nx']}x{case['ny']}x{case['nz']} periodic crop of BASELINE config {args.config} "
+                       f"(full size {full['nx']}x{full['ny']}x{full['nz']}); " + cfg["workload"].split(": ", 1)[1])
+    cfg["sample_of"] = f"config {args.config}"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": spp * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
@@ -175,6 +179,52 @@ def run_reference(args):
             "gpu_launches": 0}
     print(json.dumps(line))
     return 0
+
+
+def median(xs):
+    xs = sorted(xs)
+    return xs[len(xs) // 2]
+
+
+def time_config(binding, wl, torch, config, steps, warmup, repeats, graph, device):
+    """One configuration, device-resident: median over `repeats` of the CUDA-event time of `steps` steps, the state
+    reset before every repeat; on a side stream so that the CUDA-graph option can capture."""
+    case = wl.make_case(config)
+    cells = case["nx"] * case["ny"] * case["nz"]
+    dyc = binding.Dycore(case, device=device)
+    if graph:
+        dyc.set_option(binding.ERF_OPT_GRAPH, 1)
+    dev = [torch.from_numpy(a).to(device) for a in case["state"]]
+    side = torch.cuda.Stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    times = []
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        for rep in range(repeats):
+            dyc.set_state(*dev)
+            for _ in range(warmup if rep == 0 else 1):
+                dyc.rk3_step(case["dt"], case["ns"])
+            n0 = dyc.launch_count
+            e0.record()
+            for _ in range(steps):
+                dyc.rk3_step(case["dt"], case["ns"])
+            e1.record()
+            side.synchronize()
+            times.append(e0.elapsed_time(e1) / steps)
+            launches = (dyc.launch_count - n0) // steps
+    ms = median(times)
+    ad = algorithmic_doubles(case)
+    peak, _ = measured_peak_gbs()
+    out = {"config": config, "grid": f"{case['nx']}x{case['ny']}x{case['nz']}", "cells": cells, "ms_per_step": ms,
+           "value": cells / (ms * 1e-3), "launches_per_step": launches, "launch": "cuda_graph" if graph else "stream",
+           "algorithmic_bytes_per_cell": ad["total"] * 8,
+           "whole_step_frac": ad["total"] * 8 * cells / (ms * 1e-3) / 1e9 / peak,
+           "path": "fused flat kernels" if case.get("z_nodes") is None else "terrain: general slow RHS + fused terrain substeps",
+           "repeats": repeats, "steps": steps, "device_bytes": dyc.device_bytes}
+    dyc.close()
+    del dev
+    torch.cuda.empty_cache()
+    return out
 
 
 # ----------------------------------------------------------------------------- our arm
@@ -215,23 +265,34 @@ def run_ours(args):
     for _ in range(max(args.warmup, 0)):
         dyc.rk3_step(dt, ns)
     barrier()
-    # ---- device-resident timing: K steps, CUDA events on the launching (current) stream
+    # ---- device-resident timing: K steps, CUDA events on the launching (current) stream, no per-kernel events
+    # inside the timed region; median of `repeats` such measurements, the state reset before each
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = []
+    with ClockSampler(local) as clk:
+        for rep in range(max(args.repeats, 1)):
+            dyc.set_state(*dev)
+            dyc.rk3_step(dt, ns)
+            barrier()
+            n0 = dyc.launch_count
+            e0.record()
+            for _ in range(args.steps):
+                dyc.rk3_step(dt, ns)
+            e1.record()
+            barrier()
+            reps.append(max_over_ranks(e0.elapsed_time(e1), dist, "cuda"))
+            launches = dyc.launch_count - n0
+    ms = median(reps)
+    value = aggregate_value(world, cells, args.steps, ms)
+    # ---- per-kernel-class device times: a separate pass with the library's own event brackets switched on
     dyc.set_timing(True)
     dyc.reset_timing()
-    n0 = dyc.launch_count
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local) as clk:
-        e0.record()
-        for _ in range(args.steps):
-            dyc.rk3_step(dt, ns)
-        e1.record()
-        barrier()
-    ms = e0.elapsed_time(e1)
-    launches = dyc.launch_count - n0
+    for _ in range(args.steps):
+        dyc.rk3_step(dt, ns)
+    barrier()
     kt = dyc.timing()
     dyc.set_timing(False)
-    ms = max_over_ranks(ms, dist, "cuda")
-    value = aggregate_value(world, cells, args.steps, ms)
+    kt_steps = args.steps
 
     # ---- end to end: host buffers in, host buffers out, every step.  Every step copies its inputs from pinned host
     # memory and reads its result back; the steps are independent requests, so the copy-in of step n+1, the compute of
@@ -285,7 +346,30 @@ def run_ours(args):
     wall = time.perf_counter() - t0
     e2e_ms = max(e0.elapsed_time(e1), wall * 1e3)
     e2e_ms = max_over_ranks(e2e_ms, dist, "cuda")
-    e2e_value = aggregate_value(world, cells, e2e_steps, e2e_ms)
+    e2e_pipelined = aggregate_value(world, cells, e2e_steps, e2e_ms)
+
+    # the same end to end with NO overlap: copy in, set_state, step, get_state, copy out, one after the other on one
+    # stream -- what a time stepper whose next input is the previous output would see if it round-tripped every step
+    def e2e_serial(n):
+        for _ in range(n):
+            for d, h in zip(in_dev[0], host):
+                d.copy_(h, non_blocking=True)
+            dyc.set_state(*in_dev[0])
+            dyc.rk3_step(dt, ns)
+            dyc.get_state(out_dev[0])
+            for h, d in zip(out_host, out_dev[0]):
+                h.copy_(d, non_blocking=True)
+
+    e2e_serial(1)
+    barrier()
+    t0 = time.perf_counter()
+    e0.record()
+    e2e_serial(e2e_steps)
+    e1.record()
+    barrier()
+    wall = time.perf_counter() - t0
+    ser_ms = max_over_ranks(max(e0.elapsed_time(e1), wall * 1e3), dist, "cuda")
+    e2e_value = aggregate_value(world, cells, e2e_steps, ser_ms)
     checksum = float(out_host[4].sum())
     assert np.isfinite(checksum), "state blew up"
 
@@ -297,6 +381,7 @@ def run_ours(args):
     # ---- roofline of the dominant kernel class (device events recorded inside the library)
     peak, peak_src = measured_peak_gbs()
     ad = algorithmic_doubles(case)
+    dev_bytes = dyc.device_bytes
     alg_bytes = {"acoustic": ad["substep"] * 8 * cells, "slow_rhs": ad["slow"] * 8 * cells}
     dom = max(kt.items(), key=lambda kv: kv[1][1]) if kt else None
     roof = None
@@ -314,11 +399,12 @@ def run_ours(args):
                 "frac": achieved / peak, "traffic": measured_traffic(name, args.config), "peak_source": peak_src,
                 "launch_unit": units, "algorithmic_bytes_per_launch": per_launch,
                 "avg_launch_ms": tot_ms / calls,
-                "share_of_step": tot_ms / ms,
+                "share_of_step": (tot_ms / kt_steps) / (ms / args.steps),
                 "whole_step": {"algorithmic_bytes_per_cell": ad["total"] * 8,
                                "achieved": ad["total"] * 8 * cells * args.steps / (ms * 1e-3) / 1e9,
                                "frac": ad["total"] * 8 * cells * args.steps / (ms * 1e-3) / 1e9 / peak},
-                "kernel_ms_per_step": {k: v[1] / args.steps for k, v in kt.items()}}
+                "kernel_ms_per_step": {k: v[1] / kt_steps for k, v in kt.items()},
+                "kernel_times_from": "a separate pass of the same steps with per-kernel CUDA events on"}
 
     if roof is not None:
         # the fp64 FMA peak of this device, measured by the library's DFMA micro-benchmark; the fp64-pipe
@@ -329,6 +415,25 @@ def run_ours(args):
             roof["fp64_peak_tflops"] = None
             print(f"bench.py: fp64 peak not measured: {e}", file=sys.stderr)
 
+    # ---- the other four BASELINE configurations (north_star: throughput on all five), a few seconds in total;
+    # configs 1-2 are launch-bound: stream launches and the captured CUDA graph side by side
+    all_cfg = None
+    if world == 1 and args.config == 5 and not args.no_all_configs:
+        dyc.close()
+        del in_dev, out_dev, dev
+        torch.cuda.empty_cache()
+        all_cfg = []
+        for cfgn, kw in ((1, dict(steps=20, warmup=5)), (2, dict(steps=10, warmup=3)), (3, dict(steps=5, warmup=3)),
+                         (4, dict(steps=3, warmup=2))):
+            all_cfg.append(time_config(binding, wl, torch, cfgn, repeats=5, graph=False, device=f"cuda:{local}", **kw))
+            if cfgn <= 2:
+                all_cfg.append(time_config(binding, wl, torch, cfgn, repeats=5, graph=True, device=f"cuda:{local}", **kw))
+        all_cfg.append({"config": 5, "grid": f"{case['nx']}x{case['ny']}x{case['nz']}", "cells": cells,
+                        "ms_per_step": ms / args.steps, "value": value, "launches_per_step": launches // args.steps,
+                        "launch": "stream", "algorithmic_bytes_per_cell": ad["total"] * 8,
+                        "whole_step_frac": roof["whole_step"]["frac"] if roof else None, "path": "fused flat kernels",
+                        "repeats": max(args.repeats, 1), "steps": args.steps})
+
     # ---- the oracle beside it, on a bounded sample (rank 0, N = 1 only)
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
@@ -338,17 +443,23 @@ def run_ours(args):
     cfg = config_desc(case, args.config)
     cfg.update({"l2": "inputs larger than L2 (every field >= 1 GB)" if cells * 8 > 256e6 else
                 "fields fit in L2 (small configuration)",
-                "replicas": world, "device_bytes": dyc.device_bytes,
+                "replicas": world, "device_bytes": dev_bytes, "repeats": max(args.repeats, 1),
+                "ms_per_step_repeats": [r / args.steps for r in reps],
                 "path": "general" if args.path == 1 else "auto"})
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg, "clocks": clk.summary(),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps,
-                    "overlap": "copy-in of step n+1, compute of step n and copy-out of step n-1 on three streams"},
-            "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu}
+                    "steps": e2e_steps, "ms_per_step": ser_ms / e2e_steps, "serial_ms_per_step": ser_ms / e2e_steps,
+                    "mode": "serial: copy in, set_state, step, get_state, copy out one after the other, every step",
+                    "pipelined_independent_requests": {
+                        "value": e2e_pipelined, "ms_per_step": e2e_ms / e2e_steps,
+                        "note": "copy-in of request n+1, compute of request n and copy-out of request n-1 on three "
+                                "streams: valid for independent one-step requests, not for a time stepper"}},
+            "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu, "all_configs": all_cfg}
     print(json.dumps(line))
-    dyc.close()
+    if all_cfg is None:
+        dyc.close()
     if dist is not None:
         dist.destroy_process_group()
     return 0
@@ -363,6 +474,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", type=int, default=0, choices=[0, 1], help="0 auto (fused), 1 general kernels")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-all-configs", action="store_true", help="skip the configs 1-4 summary of the default run")
+    ap.add_argument("--repeats", type=int, default=5, help="timed repeats of the K steps (median reported)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

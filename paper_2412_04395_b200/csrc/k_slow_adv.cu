@@ -43,7 +43,7 @@ constexpr int NCOPY = TH + 4 * (TH - 2);                          // row copies 
 constexpr int NTAB = 8;                                           // per-level tables staged in shared memory
 constexpr int MAXLEV = 320;                                       // nz + 1 <= MAXLEV (shared-memory budget)
 constexpr size_t smem_bytes(int nlev) {
-  return (size_t)(NS * RAW + NPB * PB + NTAB * nlev) * sizeof(double) + NS * sizeof(uint64_t);
+  return (size_t)(NS * RAW + NPB * PB + NTAB * nlev) * sizeof(double) + (NS + 1) * sizeof(uint64_t);
 }
 
 struct Maps {
@@ -121,6 +121,7 @@ __device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const
   if (GRP == 0 && tid == 0) {
 #pragma unroll
     for (int s = 0; s < NS; s++) mbar_init(&full[s], 1);
+    mbar_init(&full[NS], NTH);  // "everybody has finished the previous iteration"
     mbar_fence_init();
   }
   cta_sync();
@@ -224,11 +225,11 @@ __device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const
     }
   };
 
-  // ---- prologue: levels Ls-1 (for rho below the first face) .. Ls+2
+  // ---- prologue: levels Ls-1 (for rho below the first face) .. Ls+1
   int sP = Ls % NS;  // raw slot of level P
   {
     const int lo = max(Ls - 1, 0);
-    for (int lv = lo; lv <= min(Ls + 2, Ld); lv++) issue(lv, lv % NS);
+    for (int lv = lo; lv <= min(Ls + 1, Ld); lv++) issue(lv, lv % NS);
     if (Ls >= 1) wait_slot((Ls - 1) % NS);
   }
   int bP = Ls % NPB;  // primitive buffer of level P
@@ -247,19 +248,19 @@ __device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const
   double fb0 = 0.0, fb1 = 0.0;                                       // vertical fluxes carried from the face below
   double U_cm = 0.0, U_pm = 0.0, V_cm = 0.0, V_pm = 0.0, pp_m = 0.0, rp_m = 0.0;  // group 0, rho*w: level L-1
 
-  // One iteration: primitives of the level that has just landed (P), then the column work two levels below
-  // (front level L = P-2, whose primitives were finished two iterations ago), ONE barrier, then the refill of the
-  // raw slot that the front level has just released.  The two halves of an iteration touch different buffers, so
-  // they overlap freely within and across warps.
+  // One iteration = the column work of the front level L = P-2 (its primitives were finished two iterations ago),
+  // then the primitives of level P, which has landed in the meantime.  The only synchronisation is a split
+  // barrier: every thread ARRIVES at the end of its iteration and WAITS for the others only between its own column
+  // work and the primitives (the first point where it overwrites something the others may still read), so warps
+  // drift up to half an iteration apart instead of stopping together at every level.  Behind that wait thread 0
+  // refills the raw slot that the previous iteration released (level P+2 takes the slot of level P-3).
+  uint64_t *const done = &full[NS];
+  unsigned done_phase = 0;
 #pragma unroll 1
   for (int P = Ls; P <= Lf + 2; P++) {
     const int sM = sP == 0 ? NS - 1 : sP - 1;        // raw slot of level P-1
     const int sL = sM == 0 ? NS - 1 : sM - 1;        // raw slot of level P-2 (= the front level L)
     const int bL = bP == NPB - 1 ? 0 : bP + 1;       // (P-2) % 3 == (P+1) % 3
-    if (P <= Ld) {
-      wait_slot(sP);
-      prim_phase(P, raw + sP * RAW, raw + sM * RAW, prim + bP * PB);
-    }
     const int L = P - 2;
     if (L >= Ls && act) {
     const double *__restrict__ r = raw + sL * RAW;
@@ -361,8 +362,16 @@ __device__ __forceinline__ void march(const SlowFlat &p, const Poly &poly, const
       f1[0] = f1[1]; f1[1] = f1[2]; f1[2] = HV;
     }
     }
-    cta_sync();
-    if (P + 3 <= Ld) issue(P + 3, sL);               // level P+3 takes the slot of level P-2
+    if (P > Ls) {                                    // everybody has finished iteration P-1
+      mbar_wait(done, done_phase);
+      done_phase ^= 1u;
+    }
+    if (P + 2 <= Ld) issue(P + 2, sL == 0 ? NS - 1 : sL - 1);  // level P+2 takes the slot of level P-3
+    if (P <= Ld) {
+      wait_slot(sP);
+      prim_phase(P, raw + sP * RAW, raw + sM * RAW, prim + bP * PB);
+    }
+    mbar_arrive(done);
     sP = sP == NS - 1 ? 0 : sP + 1;
     bP = bL;
   }
@@ -409,7 +418,7 @@ void launch_slow_adv(erf_ctx *c, const SlowFlat &pin, cudaStream_t st) {
   const int gx = (c->nx + TX - 1) / TX, gy = (c->ny + TY - 1) / TY;
   // level chunks so that a small grid still gives every SM a CTA (each chunk recomputes 6 levels)
   int nch = (2 * 148 + gx * gy - 1) / (gx * gy);
-  const int maxch = c->nz / 16 > 1 ? c->nz / 16 : 1;
+  const int maxch = c->nz / 4 > 1 ? c->nz / 4 : 1;
   if (nch > maxch) nch = maxch;
   const int kchunk = (c->nz + nch - 1) / nch;
   dim3 grid(gx, gy, (c->nz + kchunk - 1) / kchunk);
