@@ -56,6 +56,8 @@ struct erfo_ctx {
   double *rho0, *Th0, *p0, *pi0;
   /* state at time level n */
   double *S[5];
+  /* one transported scalar rho*phi (Eq. 4); NULL until erfo_set_scalar */
+  double *Q;
 };
 
 /* ------------------------------------------------------------------ */
@@ -833,6 +835,9 @@ typedef struct {
   double *P[5];                        /* S'' = (rho'', U'', V'', W'', Theta'') */
   double *Om;                          /* Omega'' at the end of the previous substep */
   double *Th_prev;                     /* Theta'' one substep back (divergence damping) */
+  /* sums over the substeps of the perturbation momenta that advance rho'' (L138: "the time average over the
+   * RK stage of the intermediate (rho u . n) values used to advance rho each substep"); NULL = not wanted */
+  double *Usum, *Vsum, *Omsum;
 } acoustic_t;
 
 /* coefficients of row k (1..nz-1) of the column system for Omega''^{new}.
@@ -899,6 +904,11 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
       }
   fill_periodic(c, Upp);
   fill_periodic(c, Vpp);
+  if (ac->Usum) /* the horizontal momenta that enter this substep's continuity equation (step 4) */
+    for (size_t a = 0; a < c->n; a++) {
+      ac->Usum[a] += Upp[a];
+      ac->Vsum[a] += Vpp[a];
+    }
 
   /* 3. explicit slope part of W'': omega = sxw avg4(U''new) + syw avg4(V''new) [R:G16] */
   double *om = fnew(c);
@@ -982,6 +992,9 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
         Tpp[a] = Ttil[k] - dtau * b2 * (thf[k + 1] * On[k + 1] - thf[k] * On[k]) / hc;
         rpp[a] = rtil[k] - dtau * b2 * (On[k + 1] - On[k]) / hc;
       }
+      /* the vertical flux that advanced rho'' in this substep: beta2 Omega''new + beta1 Omega''old (L591) */
+      if (ac->Omsum)
+        for (int k = 0; k <= nz; k++) ac->Omsum[IX(c, i, j, k)] += b2 * On[k] + b1 * ac->Om[IX(c, i, j, k)];
       for (int k = 0; k <= nz; k++) ac->Om[IX(c, i, j, k)] = On[k];
     }
   free(Ttil); free(rtil); free(That); free(rhat); free(thf);
@@ -998,8 +1011,13 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
 /* run n substeps from S'' (ghosts filled) about stage state St */
 static void acoustic_loop(const erfo_ctx *c, double *const St[5], const double *theta_t,
                           const double *pi_t, double *const R[5], double *P[5], double dtau,
-                          int n) {
+                          int n, double *Mavg[3]) {
   acoustic_t ac;
+  ac.Usum = Mavg ? Mavg[0] : NULL;
+  ac.Vsum = Mavg ? Mavg[1] : NULL;
+  ac.Omsum = Mavg ? Mavg[2] : NULL;
+  if (Mavg)
+    for (int m = 0; m < 3; m++) memset(Mavg[m], 0, c->n * sizeof(double));
   ac.theta_t = theta_t;
   ac.pi_t = pi_t;
   ac.Th_t = St[TH];
@@ -1010,8 +1028,123 @@ static void acoustic_loop(const erfo_ctx *c, double *const St[5], const double *
   contravariant_flux(c, P[UU], P[VV], P[WW], ac.Om); /* Omega'' of the initial S'' */
   memcpy(ac.Th_prev, P[TH], c->n * sizeof(double));  /* Theta''_prev = Theta'' */
   for (int s = 0; s < n; s++) acoustic_substep(c, &ac, dtau);
+  if (Mavg) /* sums -> time averages over the stage */
+    for (int m = 0; m < 3; m++) {
+      for (size_t a = 0; a < c->n; a++) Mavg[m][a] /= (double)n;
+      fill_periodic(c, Mavg[m]);
+    }
   free(ac.Om);
   free(ac.Th_prev);
+}
+
+/* ------------------------------------------------------------------ */
+/* Eq. 4: one transported scalar (L69), advanced after the substeps    */
+/* (L138)                                                              */
+/* ------------------------------------------------------------------ */
+
+/* Q_stage = Q^n + dts * [ -div(Mbar phi^t) + div(K grad phi^t) ],  phi^t = Q^t / rho^t.
+ * Mbar = (Ub, Vb, Omb): the stage-time-averaged normal momenta (stage momenta + averaged perturbations), so
+ * that the scalar sees exactly the mass fluxes that advanced rho in the substeps (L138) -- a constant phi then
+ * stays constant.  Interpolation of phi as for theta (Eq. 17-21 with the sign of Mbar; order reduction at the
+ * lids [R:G13]).  Diffusion as for theta, conservative form, with the same diffusivity K = rho alpha (+ mu_t/Pr_t)
+ * evaluated at the stage state [R:G25]. */
+static void scalar_stage(const erfo_ctx *c, double *const St[5], const double *Qt, const double *Qn,
+                         const double *Ub, const double *Vb, const double *Omb, double dts, double *Qout) {
+  int nx = c->nx, ny = c->ny, nz = c->nz;
+  int oh = c->p.adv_order_h, ov = c->p.adv_order_v;
+  double dx = c->dx, dy = c->dy;
+  double *phi = fnew(c), *Fx = fnew(c), *Fy = fnew(c), *R = fnew(c);
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < nz; k++)
+    for (int j = 0; j < ny; j++)
+      for (int i = 0; i < nx; i++) {
+        size_t a = IX(c, i, j, k);
+        phi[a] = Qt[a] / St[RHO][a];
+        Fx[a] = c->hx[a] * Ub[a];
+        Fy[a] = c->hy[a] * Vb[a];
+      }
+  fill_periodic(c, phi);
+  fill_periodic(c, Fx);
+  fill_periodic(c, Fy);
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < nz; k++)
+    for (int j = 0; j < ny; j++)
+      for (int i = 0; i < nx; i++) {
+        size_t a = IX(c, i, j, k);
+        double fxm = Fx[a], fxp = Fx[IX(c, i + 1, j, k)];
+        double fym = Fy[a], fyp = Fy[IX(c, i, j + 1, k)];
+        double omm = Omb[a], omp = Omb[IX(c, i, j, k + 1)];
+        double txm = fxm * interp_x(c, phi, i, j, k, oh, fxm);
+        double txp = fxp * interp_x(c, phi, i + 1, j, k, oh, fxp);
+        double tym = fym * interp_y(c, phi, i, j, k, oh, fym);
+        double typ = fyp * interp_y(c, phi, i, j + 1, k, oh, fyp);
+        double tzm = (k >= 1) ? omm * interp_z(c, phi, i, j, k, 0, nz - 1, ov, omm) : 0.0;
+        double tzp = (k + 1 <= nz - 1) ? omp * interp_z(c, phi, i, j, k + 1, 0, nz - 1, ov, omp) : 0.0;
+        R[a] = -((txp - txm) / dx + (typ - tym) / dy + (tzp - tzm)) / c->hc[a];
+      }
+  if (c->p.diffusion != 0) {
+    prim_t q;
+    q.theta = fnew(c); q.pp = fnew(c); q.pi = fnew(c);
+    q.u = fnew(c); q.v = fnew(c); q.w = fnew(c);
+    primitives(c, St, &q);
+    diff_t d;
+    d.mu = fnew(c); d.K = fnew(c);
+    d.S11 = fnew(c); d.S22 = fnew(c); d.S33 = fnew(c);
+    d.S12 = fnew(c); d.S13 = fnew(c); d.S23 = fnew(c);
+    d.qu = fnew(c); d.qv = fnew(c);
+    strain_and_viscosity(c, St, &q, &d);
+    double *qph = fnew(c), *Gx = fnew(c), *Gy = fnew(c), *Gz = fnew(c);
+    for (int k = 1; k < nz; k++)
+      for (int j = 0; j < ny; j++)
+        for (int i = 0; i < nx; i++) {
+          size_t a = IX(c, i, j, k);
+          qph[a] = (phi[a] - phi[IX(c, i, j, k - 1)]) / c->hw[a];
+        }
+    fill_periodic(c, qph);
+    for (int k = 0; k < nz; k++)
+      for (int j = 0; j < ny; j++)
+        for (int i = 0; i < nx; i++) {
+          size_t a = IX(c, i, j, k);
+          size_t z0 = IX(c, i, j, 0), zim = IX(c, i - 1, j, 0), zjm = IX(c, i, j - 1, 0);
+          double Kx = 0.5 * (d.K[IX(c, i - 1, j, k)] + d.K[a]);
+          double Ky = 0.5 * (d.K[IX(c, i, j - 1, k)] + d.K[a]);
+          double dpx = (phi[a] - phi[IX(c, i - 1, j, k)]) / dx - c->sxu[a] * avg_q_valid(c, qph, zim, z0, k);
+          double dpy = (phi[a] - phi[IX(c, i, j - 1, k)]) / dy - c->syv[a] * avg_q_valid(c, qph, zjm, z0, k);
+          Gx[a] = -Kx * dpx;
+          Gy[a] = -Ky * dpy;
+        }
+    fill_periodic(c, Gx);
+    fill_periodic(c, Gy);
+    for (int k = 1; k < nz; k++)
+      for (int j = 0; j < ny; j++)
+        for (int i = 0; i < nx; i++) {
+          size_t a = IX(c, i, j, k);
+          double Kw = 0.5 * (d.K[IX(c, i, j, k - 1)] + d.K[a]);
+          double gxb = 0.25 * (Gx[IX(c, i, j, k - 1)] + Gx[IX(c, i + 1, j, k - 1)] + Gx[a] + Gx[IX(c, i + 1, j, k)]);
+          double gyb = 0.25 * (Gy[IX(c, i, j, k - 1)] + Gy[IX(c, i, j + 1, k - 1)] + Gy[a] + Gy[IX(c, i, j + 1, k)]);
+          Gz[a] = -Kw * qph[a] - c->sxw[a] * gxb - c->syw[a] * gyb;
+        } /* Gz = 0 on the lids */
+    for (int k = 0; k < nz; k++)
+      for (int j = 0; j < ny; j++)
+        for (int i = 0; i < nx; i++) {
+          size_t a = IX(c, i, j, k);
+          size_t ip = IX(c, i + 1, j, k), jp = IX(c, i, j + 1, k), kp = IX(c, i, j, k + 1);
+          R[a] -= ((c->hx[ip] * Gx[ip] - c->hx[a] * Gx[a]) / dx + (c->hy[jp] * Gy[jp] - c->hy[a] * Gy[a]) / dy +
+                   (Gz[kp] - Gz[a])) / c->hc[a];
+        }
+    free(qph); free(Gx); free(Gy); free(Gz);
+    free(d.mu); free(d.K); free(d.S11); free(d.S22); free(d.S33);
+    free(d.S12); free(d.S13); free(d.S23); free(d.qu); free(d.qv);
+    free(q.theta); free(q.pp); free(q.pi); free(q.u); free(q.v); free(q.w);
+  }
+  for (int k = 0; k < nz; k++)
+    for (int j = 0; j < ny; j++)
+      for (int i = 0; i < nx; i++) {
+        size_t a = IX(c, i, j, k);
+        Qout[a] = Qn[a] + dts * R[a];
+      }
+  fill_periodic(c, Qout);
+  free(phi); free(Fx); free(Fy); free(R);
 }
 
 /* ------------------------------------------------------------------ */
@@ -1031,19 +1164,41 @@ int erfo_rk3_step(erfo_ctx *c, double dt, int n_acoustic) {
   for (int m = 0; m < 5; m++) { St[m] = fnew(c); R[m] = fnew(c); P[m] = fnew(c); }
   double *theta_t = fnew(c), *pi_t = fnew(c);
   for (int m = 0; m < 5; m++) memcpy(St[m], c->S[m], c->n * sizeof(double)); /* S^t = S^n */
+  /* transported scalar: stage value Q^t, time-averaged momenta of the stage */
+  double *Qt = NULL, *Qnew = NULL, *Mavg[3] = {NULL, NULL, NULL}, *Omt = NULL;
+  if (c->Q) {
+    Qt = fnew(c); Qnew = fnew(c); Omt = fnew(c);
+    for (int m = 0; m < 3; m++) Mavg[m] = fnew(c);
+    memcpy(Qt, c->Q, c->n * sizeof(double));
+  }
   for (int stage = 1; stage <= 3; stage++) {
     int nsub; double dtau, dts;
     erfo_schedule(stage, dt, n_acoustic, &nsub, &dtau, &dts);
     slow_rhs(c, St, R, theta_t, pi_t); /* f(S^t), recomputed every stage (L140) */
     if (c->p.substep_mode == 0) {
       /* no substepping (L140): S_stage = S^n + dts * f(S^t) */
+      if (c->Q) { /* no substepping: the stage momenta themselves advect the scalar */
+        contravariant_flux(c, St[UU], St[VV], St[WW], Omt);
+        scalar_stage(c, St, Qt, c->Q, St[UU], St[VV], Omt, dts, Qnew);
+        memcpy(Qt, Qnew, c->n * sizeof(double));
+      }
       for (int m = 0; m < 5; m++)
         for (size_t a = 0; a < c->n; a++) St[m][a] = c->S[m][a] + dts * R[m][a];
     } else {
       /* perturbation about the most recent stage (L581); every stage starts from S^n [R:G7] */
       for (int m = 0; m < 5; m++)
         for (size_t a = 0; a < c->n; a++) P[m][a] = c->S[m][a] - St[m][a];
-      acoustic_loop(c, St, theta_t, pi_t, R, P, dtau, nsub);
+      acoustic_loop(c, St, theta_t, pi_t, R, P, dtau, nsub, c->Q ? Mavg : NULL);
+      if (c->Q) { /* Eq. 4 after the substeps (L138): averaged momenta = stage momenta + averaged perturbations */
+        contravariant_flux(c, St[UU], St[VV], St[WW], Omt);
+        for (size_t a = 0; a < c->n; a++) {
+          Mavg[0][a] += St[UU][a];
+          Mavg[1][a] += St[VV][a];
+          Mavg[2][a] += Omt[a];
+        }
+        scalar_stage(c, St, Qt, c->Q, Mavg[0], Mavg[1], Mavg[2], dts, Qnew);
+        memcpy(Qt, Qnew, c->n * sizeof(double));
+      }
       for (int m = 0; m < 5; m++) /* L593 */
         for (size_t a = 0; a < c->n; a++) St[m][a] = St[m][a] + P[m][a];
     }
@@ -1053,6 +1208,11 @@ int erfo_rk3_step(erfo_ctx *c, double dt, int n_acoustic) {
   for (int m = 0; m < 5; m++) memcpy(c->S[m], St[m], c->n * sizeof(double));
   for (int m = 0; m < 5; m++) { free(St[m]); free(R[m]); free(P[m]); }
   free(theta_t); free(pi_t);
+  if (c->Q) {
+    memcpy(c->Q, Qt, c->n * sizeof(double));
+    free(Qt); free(Qnew); free(Omt);
+    for (int m = 0; m < 3; m++) free(Mavg[m]);
+  }
   return 0;
 }
 
@@ -1114,6 +1274,7 @@ void erfo_destroy(erfo_ctx *c) {
                    c->sxw, c->syw, c->sxu, c->syv, c->rho0, c->Th0, c->p0, c->pi0,
                    c->S[0], c->S[1], c->S[2], c->S[3], c->S[4]};
   for (size_t a = 0; a < sizeof(all) / sizeof(all[0]); a++) free(all[a]);
+  free(c->Q);
   free(c);
 }
 
@@ -1126,6 +1287,20 @@ int erfo_set_state(erfo_ctx *c, const double *rho, const double *rhou, const dou
   put_dense(c, c->S[WW], rhow, c->nz + 1);
   put_dense(c, c->S[TH], rhotheta, c->nz);
   impose_lids(c, c->S[UU], c->S[VV], c->S[WW]);
+  return 0;
+}
+
+/* Eq. 4 (L69): give the context one transported scalar, as rho*phi [nz][ny][nx]; erfo_rk3_step then advances it */
+int erfo_set_scalar(erfo_ctx *c, const double *rhophi) {
+  if (!c || !rhophi) return -1;
+  if (!c->Q) c->Q = fnew(c);
+  put_dense(c, c->Q, rhophi, c->nz);
+  return 0;
+}
+
+int erfo_get_scalar(erfo_ctx *c, double *rhophi) {
+  if (!c || !rhophi || !c->Q) return -1;
+  get_dense(c, c->Q, rhophi, c->nz);
   return 0;
 }
 
@@ -1206,7 +1381,7 @@ int erfo_acoustic(erfo_ctx *c, double dtau, int n, const double *R_rho, const do
   q.theta = fnew(c); q.pp = fnew(c); q.pi = fnew(c);
   q.u = fnew(c); q.v = fnew(c); q.w = fnew(c);
   primitives(c, c->S, &q);
-  acoustic_loop(c, c->S, q.theta, q.pi, R, P, dtau, n);
+  acoustic_loop(c, c->S, q.theta, q.pi, R, P, dtau, n, NULL);
   get_dense(c, P[RHO], rho_pp, c->nz); get_dense(c, P[UU], U_pp, c->nz);
   get_dense(c, P[VV], V_pp, c->nz); get_dense(c, P[WW], W_pp, c->nz + 1);
   get_dense(c, P[TH], Theta_pp, c->nz);

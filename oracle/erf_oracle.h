@@ -61,6 +61,11 @@ int erfo_get_state(erfo_ctx *, double *rho, double *rhou, double *rhov, double *
                    double *rhotheta);
 void erfo_destroy(erfo_ctx *);
 
+/* One transported scalar rho*phi [nz][ny][nx] (Eq. 4).  Once set, erfo_rk3_step advances it in every
+ * RK stage AFTER the acoustic substeps, with the stage-time-averaged normal momenta (L138). */
+int erfo_set_scalar(erfo_ctx *, const double *rhophi);
+int erfo_get_scalar(erfo_ctx *, double *rhophi);
+
 /* ---- per-operator entry points used by the pinning tests ---- */
 
 /* Eq. 17-21 interpolant at the flux point between q[2]=q_{m-1} and q[3]=q_m;

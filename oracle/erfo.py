@@ -78,6 +78,8 @@ def lib():
         L.erfo_set_state.argtypes = [C.c_void_p] + [_dp] * 5
         L.erfo_get_state.argtypes = [C.c_void_p] + [_dp] * 5
         L.erfo_rk3_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
+        L.erfo_set_scalar.argtypes = [C.c_void_p, _dp]
+        L.erfo_get_scalar.argtypes = [C.c_void_p, _dp]
         L.erfo_destroy.argtypes = [C.c_void_p]
         L.erfo_destroy.restype = None
         L.erfo_interp.argtypes = [C.c_int, C.c_double, _dp]
@@ -172,6 +174,16 @@ class Oracle:
                np.empty(self.shape_w), np.empty(self.shape_c)]
         rc = self._L.erfo_get_state(self._h, *[_p(x) for x in out])
         assert rc == 0
+        return out
+
+    def set_scalar(self, rhophi):
+        a = _c(rhophi)
+        assert a.shape == self.shape_c
+        assert self._L.erfo_set_scalar(self._h, _p(a)) == 0
+
+    def get_scalar(self):
+        out = np.empty(self.shape_c)
+        assert self._L.erfo_get_scalar(self._h, _p(out)) == 0
         return out
 
     def step(self, dt, n_acoustic):
