@@ -25,7 +25,7 @@ ERF_VARIANT_ZC_WIDE, ERF_VARIANT_FORCE_ZC, ERF_VARIANT_DIFF_SPLIT = 16, 32, 1024
 ERF_VARIANT_FORCE_COLUMN, ERF_VARIANT_SPLIT_SLOW_RHS = 4096, 8192
 
 EXPORTS = ["erf_create", "erf_set_state", "erf_rk3_step", "erf_get_state", "erf_destroy",
-           "erf_strerror", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_set_option", "erf_launch_count",
+           "erf_strerror", "erf_set_scalar", "erf_get_scalar", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_set_option", "erf_launch_count",
            "erf_device_bytes", "erf_set_timing", "erf_get_timing", "erf_reset_timing", "erf_timing_name",
            "erf_measure_fp64_peak"]
 ERF_TIMING_CLASSES = 8
@@ -83,6 +83,8 @@ def load(path: str | None = None):
     L.erf_strerror.restype = C.c_char_p
     L.erf_slow_rhs.argtypes = [C.c_void_p] + [_dp] * 5 + [C.c_void_p]
     L.erf_acoustic.argtypes = [C.c_void_p, C.c_double, C.c_int] + [_dp] * 10 + [C.c_void_p]
+    L.erf_set_scalar.argtypes = [C.c_void_p, _dp, C.c_void_p]
+    L.erf_get_scalar.argtypes = [C.c_void_p, _dp, C.c_void_p]
     L.erf_set_path.argtypes = [C.c_void_p, C.c_int]
     L.erf_set_option.argtypes = [C.c_void_p, C.c_int, C.c_longlong]
     L.erf_launch_count.argtypes = [C.c_void_p]
@@ -142,6 +144,14 @@ def erf_rk3_step(h, dt, n_acoustic, stream=None):
 def erf_get_state(h, rho, rhou, rhov, rhow, rhotheta, stream=None):
     _ck(load().erf_get_state(h, _ptr(rho), _ptr(rhou), _ptr(rhov), _ptr(rhow), _ptr(rhotheta),
                              _stream(stream)), "erf_get_state")
+
+
+def erf_set_scalar(h, rhophi, stream=None):
+    _ck(load().erf_set_scalar(h, _ptr(rhophi), _stream(stream)), "erf_set_scalar")
+
+
+def erf_get_scalar(h, rhophi, stream=None):
+    _ck(load().erf_get_scalar(h, _ptr(rhophi), _stream(stream)), "erf_get_scalar")
 
 
 def erf_destroy(h):
@@ -272,6 +282,14 @@ class Dycore:
 
     def set_state(self, rho, U, V, W, Th, stream=None):
         erf_set_state(self._h, rho, U, V, W, Th, stream)
+
+    def set_scalar(self, rhophi, stream=None):
+        erf_set_scalar(self._h, rhophi, stream)
+
+    def get_scalar(self, stream=None):
+        out = self.empty_state()[0]
+        erf_get_scalar(self._h, out, stream)
+        return out
 
     def get_state(self, out=None, stream=None):
         out = out if out is not None else self.empty_state()

@@ -106,6 +106,8 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   c->gen_ready = false;
   c->graph_on = false;
   c->graph_warm = false;
+  c->sc_Q = c->sc_Qt = c->sc_Qnew = c->sc_phi = c->sc_R = nullptr;
+  c->sc_sum[0] = c->sc_sum[1] = c->sc_sum[2] = nullptr;
   c->base1d_r0 = c->base1d_T0 = nullptr;
   c->zxf = c->zyf = c->zw = c->hx = c->hy = c->hc = c->zc = c->hw = c->hu = c->hv = nullptr;
   c->sxw = c->syw = c->sxu = c->syv = c->rho0 = c->Th0 = c->p0 = c->pi0 = c->Om_slow = nullptr;
@@ -259,7 +261,25 @@ extern "C" const char *erf_timing_name(int id) {
 extern "C" long long erf_launch_count(const erf_ctx *c) { return c ? c->launches : 0; }
 extern "C" long long erf_device_bytes(const erf_ctx *c) { return c ? c->bytes : 0; }
 
-static bool use_fused(const erf_ctx *c) { return c->path == ERF_PATH_AUTO && fused_available(c); }
+// (a context with a transported scalar runs the terrain-general kernels, which accumulate the averaged momenta)
+static bool use_fused(const erf_ctx *c) { return c->path == ERF_PATH_AUTO && fused_available(c) && !c->sc_Q; }
+
+extern "C" int erf_set_scalar(erf_ctx *c, const double *rhophi, void *stream) {
+  if (!c || !rhophi) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (ensure_general(c, st) != ERF_OK || !ensure_scalar(c)) return c->status;
+  cudaMemcpyAsync(c->sc_Q, rhophi, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  return check(c);
+}
+
+extern "C" int erf_get_scalar(erf_ctx *c, double *rhophi, void *stream) {
+  if (!c || !rhophi || !c->sc_Q) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  cudaMemcpyAsync(rhophi, c->sc_Q, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice,
+                  (cudaStream_t)stream);
+  return check(c);
+}
 
 // substep schedule of RK stage s (L170): one substep of dt/3 in stage 1, then ns/2 and ns of dt/ns
 static void schedule(int stage, double dt, int ns, int *nsub, double *dtau, double *dts) {
@@ -332,6 +352,7 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
   if (ensure_general(c, st) != ERF_OK) return c->status;
   for (int f = 0; f < 5; f++)  // S^t = S^n
     cudaMemcpyAsync(c->St.f[f], c->S.f[f], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  if (c->sc_Q) cudaMemcpyAsync(c->sc_Qt, c->sc_Q, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
   for (int stage = 1; stage <= 3; stage++) {
     int nsub; double dtau, dts;
     schedule(stage, dt, n_acoustic, &nsub, &dtau, &dts);
@@ -340,6 +361,10 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
       general_slow_rhs(c, c->St, st);  // f(S^t), every stage (L140)
     }
     if (c->p.substep_mode == 0) {
+      if (c->sc_Q) {  // Eq. 4 with the stage momenta (L140)
+        scalar_stage(c, c->St, c->sc_Qt, c->sc_Q, c->sc_Qnew, 0, dts, st);
+        double *t = c->sc_Qt; c->sc_Qt = c->sc_Qnew; c->sc_Qnew = t;
+      }
       F5 S = c->S, St = c->St, R = c->R;
       View v = c->v;
       launch_cells(c, st, c->nz + 1, [=] __device__(int i, int j, int k) {
@@ -355,8 +380,12 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
       }
       {
         Timed t(c, T_ACOUSTIC_GENERAL, st);
-        if (c->path == ERF_PATH_AUTO && terrain_acoustic_available(c)) terrain_acoustic(c, c->St, dtau, nsub, st);
+        if (c->path == ERF_PATH_AUTO && terrain_acoustic_available(c) && !c->sc_Q) terrain_acoustic(c, c->St, dtau, nsub, st);
         else general_acoustic(c, c->St, dtau, nsub, st);
+      }
+      if (c->sc_Q) {  // Eq. 4 after the substeps of the stage (L138), before S^t becomes the stage result
+        scalar_stage(c, c->St, c->sc_Qt, c->sc_Q, c->sc_Qnew, nsub, dts, st);
+        double *t = c->sc_Qt; c->sc_Qt = c->sc_Qnew; c->sc_Qnew = t;
       }
       {
         Timed t(c, T_STAGE_GENERAL, st);
@@ -369,6 +398,7 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
     c->S.f[f] = c->St.f[f];
     c->St.f[f] = t;
   }
+  if (c->sc_Q) { double *t = c->sc_Q; c->sc_Q = c->sc_Qt; c->sc_Qt = t; }
   return check(c);
 }
 

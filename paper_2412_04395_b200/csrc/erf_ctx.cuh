@@ -49,6 +49,10 @@ struct erf_ctx {
   bool gen_ready;
   double *base1d_r0, *base1d_T0;  // flat grid, 1-D base state: owned copies of the [nz] inputs (to build the 3-D arrays later)
 
+  // one transported scalar (k_scalar.cu): rho*phi, its stage values, the sums of the substep momenta; null until
+  // erf_set_scalar
+  double *sc_Q, *sc_Qt, *sc_Qnew, *sc_sum[3], *sc_phi, *sc_R;
+
   // ERF_OPT_GRAPH: one instantiated CUDA graph per buffer configuration of the fused step
   struct StepGraph {
     std::vector<const void *> before, after;  // buffer roles when the step starts / ends
@@ -145,6 +149,11 @@ void general_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t
 void general_stage_init(erf_ctx *c, cudaStream_t st);    // P = S - St
 void general_stage_finish(erf_ctx *c, cudaStream_t st);  // St += P, lids
 void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st);
+
+// k_scalar.cu: Eq. 4 after the substeps of a stage, with the time-averaged momenta (L138)
+bool ensure_scalar(erf_ctx *c);
+void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, double *Qout, int nsub, double dts,
+                  cudaStream_t st);
 
 // k_acoustic_terrain.cu: general_acoustic with the per-substep passes fused (terrain grids)
 bool terrain_acoustic_available(const erf_ctx *c);

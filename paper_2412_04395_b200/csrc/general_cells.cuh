@@ -514,6 +514,7 @@ struct Acou {
   double *Th_prev, *Thd;                // divergence damping (L144) [R:G6]
   double *om;                           // explicit slope part of W''
   double *Ttil, *rtil, *cpr, *dpr;      // column scratch
+  double *Usum, *Vsum, *Omsum;          // sums of the momenta that advance rho'' (L138), for the scalars; may be null
 };
 
 // step 1: Theta''_d = Theta'' + beta_d (Theta'' - Theta''_prev); prev <- Theta''
@@ -530,8 +531,14 @@ ERF_HD void ac_horiz(const View &c, const Acou &A, double dtau, int i, int j, in
   double gR = c.gam * c.Rd;
   double piu = 0.5 * (A.pi_t[IX(c, i - 1, j, k)] + A.pi_t[a]);
   double piv = 0.5 * (A.pi_t[IX(c, i, j - 1, k)] + A.pi_t[a]);
-  A.P[UU][a] += dtau * (-gR * piu * grad_x(c, A.Thd, i, j, k) + A.R[UU][a]);
-  A.P[VV][a] += dtau * (-gR * piv * grad_y(c, A.Thd, i, j, k) + A.R[VV][a]);
+  const double Un = A.P[UU][a] + dtau * (-gR * piu * grad_x(c, A.Thd, i, j, k) + A.R[UU][a]);
+  const double Vn = A.P[VV][a] + dtau * (-gR * piv * grad_y(c, A.Thd, i, j, k) + A.R[VV][a]);
+  A.P[UU][a] = Un;
+  A.P[VV][a] = Vn;
+  if (A.Usum) {  // the horizontal momenta of this substep's continuity equation
+    A.Usum[a] += Un;
+    A.Vsum[a] += Vn;
+  }
 }
 
 // step 3: omega = sxw avg4(U''new) + syw avg4(V''new), k = 1..nz-1 [R:G16]
@@ -614,6 +621,7 @@ ERF_HD void ac_column(const View &c, const Acou &A, double dtau, int i, int j) {
     if (k >= 1) {
       On_b = A.dpr[a] - A.cpr[a] * On_t;
       A.P[WW][a] = On_b + A.om[a];
+      if (A.Omsum) A.Omsum[a] += b2 * On_b + b1 * A.Om[a];  // the vertical flux that advanced rho'' (L591)
     }
     double th = A.theta_t[a];
     double thf_b = (k >= 1) ? 0.5 * (A.theta_t[IX(c, i, j, k - 1)] + th) : 0.0;

@@ -169,6 +169,11 @@ void general_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t
     A.R[m] = c->R.f[m];
     A.P[m] = c->P.f[m];
   }
+  A.Usum = A.Vsum = A.Omsum = nullptr;
+  if (c->sc_Q) {
+    A.Usum = c->sc_sum[0]; A.Vsum = c->sc_sum[1]; A.Omsum = c->sc_sum[2];
+    for (int m = 0; m < 3; m++) cudaMemsetAsync(c->sc_sum[m], 0, c->NW * sizeof(double), st);
+  }
   // Omega'' of the initial S''; Theta''_prev = Theta''
   launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) {
     size_t a = IX(v, i, j, k);

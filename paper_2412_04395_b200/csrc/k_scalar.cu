@@ -1,0 +1,135 @@
+// k_scalar.cu -- one transported scalar rho*phi (Eq. 4).
+//
+// "Equations 4-6 do not directly participate in the substepping; these variables are advanced as if there is no
+// substepping, with the exception that the normal momenta used to define the advective fluxes is the time average
+// over the RK stage of the intermediate (rho u . n) values used to advance rho each substep" (L138).  So per stage:
+//     Q_stage = Q^n + dt_s [ -div(Mbar phi^t) + div(K grad phi^t) ],   phi^t = Q^t / rho^t,
+// Mbar = stage momenta + (1/n) sum over the substeps of (U''new, V''new, beta2 Omega''new + beta1 Omega''old) -- the
+// fluxes of the substepped continuity equation (Appendix A, L585 row 5 with L591), accumulated by the substep kernels
+// (general_cells.cuh: ac_horiz, ac_column).  With them a constant phi stays constant to round-off.  phi is interpolated
+// like theta (Eq. 17-21, order reduction at the lids [R:G13]); it diffuses with theta's K, conservative form [R:G25].
+//
+// Round 2: runs on the terrain-general data path (thread per cell, mass fluxes and vertical quotients formed on
+// the fly); a context with a scalar takes the general kernels for the whole step.
+#include "erf_ctx.cuh"
+
+namespace erfb {
+
+namespace {
+
+struct Sc {
+  View v;
+  const double *rho, *U, *V, *W;     // stage state S^t
+  const double *Us, *Vs, *Oms;       // sums over the substeps (null without substepping)
+  double rn;                         // 1 / number of substeps
+  const double *Qt, *Qn, *K;
+  double *phi, *Gx, *Gy, *R, *Qout;
+  double dts;
+};
+
+__device__ __forceinline__ double mx(const Sc &s, int i, int j, int k) {  // averaged mass flux through x-face i
+  const size_t a = IX(s.v, i, j, k);
+  return s.v.hx[a] * (s.U[a] + (s.Us ? s.rn * s.Us[a] : 0.0));
+}
+__device__ __forceinline__ double my(const Sc &s, int i, int j, int k) {
+  const size_t a = IX(s.v, i, j, k);
+  return s.v.hy[a] * (s.V[a] + (s.Vs ? s.rn * s.Vs[a] : 0.0));
+}
+__device__ __forceinline__ double mz(const Sc &s, int i, int j, int k) {  // averaged Omega through w-face k
+  if (k < 1 || k > s.v.nz - 1) return 0.0;
+  return gen::omega_at(s.v, s.U, s.V, s.W, i, j, k) + (s.Oms ? s.rn * s.Oms[IX(s.v, i, j, k)] : 0.0);
+}
+
+// mean vertical difference quotient of phi around level k at the two columns (ia, ja), (ib, jb): faces k and k+1
+// where they are interior (the chain-rule term of a horizontal derivative [R:G14])
+__device__ __forceinline__ double dz_mean(const Sc &s, int ia, int ja, int ib, int jb, int k) {
+  double sum = 0.0;
+  int n = 0;
+  for (int kk = k; kk <= k + 1; kk++)
+    if (kk >= 1 && kk <= s.v.nz - 1) {
+      const size_t a = IX(s.v, ia, ja, kk), b = IX(s.v, ib, jb, kk);
+      sum += (s.phi[a] - s.phi[IX(s.v, ia, ja, kk - 1)]) / s.v.hw[a] + (s.phi[b] - s.phi[IX(s.v, ib, jb, kk - 1)]) / s.v.hw[b];
+      n += 2;
+    }
+  return n ? sum / n : 0.0;
+}
+
+__device__ __forceinline__ double gx_at(const Sc &s, int i, int j, int k) {  // diffusive flux through x-face i
+  const size_t a = IX(s.v, i, j, k), m = IX(s.v, i - 1, j, k);
+  const double d = (s.phi[a] - s.phi[m]) / s.v.dx - s.v.sxu[a] * dz_mean(s, i - 1, j, i, j, k);
+  return -0.5 * (s.K[m] + s.K[a]) * d;
+}
+__device__ __forceinline__ double gy_at(const Sc &s, int i, int j, int k) {
+  const size_t a = IX(s.v, i, j, k), m = IX(s.v, i, j - 1, k);
+  const double d = (s.phi[a] - s.phi[m]) / s.v.dy - s.v.syv[a] * dz_mean(s, i, j - 1, i, j, k);
+  return -0.5 * (s.K[m] + s.K[a]) * d;
+}
+
+}  // namespace
+
+// Q_stage from Q^t (stage value) and Q^n; nsub = 0: no substepping (the stage momenta advect)
+void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, double *Qout, int nsub, double dts,
+                  cudaStream_t st) {
+  Sc s;
+  s.v = c->v;
+  s.rho = St.f[RHO]; s.U = St.f[UU]; s.V = St.f[VV]; s.W = St.f[WW];
+  s.Us = nsub ? c->sc_sum[0] : nullptr; s.Vs = nsub ? c->sc_sum[1] : nullptr; s.Oms = nsub ? c->sc_sum[2] : nullptr;
+  s.rn = nsub ? 1.0 / nsub : 0.0;
+  s.Qt = Qt; s.Qn = Qn; s.K = c->p.diffusion != 0 ? c->diff.K : nullptr;
+  s.phi = c->sc_phi; s.R = c->sc_R; s.Gx = c->diff.Fx; s.Gy = c->diff.Fy; s.Qout = Qout;
+  s.dts = dts;
+  const int nz = c->nz;
+  const bool diffuse = c->p.diffusion != 0;
+  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
+    const size_t a = IX(s.v, i, j, k);
+    s.phi[a] = s.Qt[a] / s.rho[a];
+  });
+  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
+    const View &v = s.v;
+    const size_t a = IX(v, i, j, k);
+    const double fxm = mx(s, i, j, k), fxp = mx(s, i + 1, j, k), fym = my(s, i, j, k), fyp = my(s, i, j + 1, k);
+    const double omm = mz(s, i, j, k), omp = mz(s, i, j, k + 1);
+    const double ax = fxp * gen::interp_x(v, s.phi, i + 1, j, k, v.oh, fxp) - fxm * gen::interp_x(v, s.phi, i, j, k, v.oh, fxm);
+    const double ay = fyp * gen::interp_y(v, s.phi, i, j + 1, k, v.oh, fyp) - fym * gen::interp_y(v, s.phi, i, j, k, v.oh, fym);
+    const double zt = (k + 1 <= v.nz - 1) ? omp * gen::interp_z(v, s.phi, i, j, k + 1, 0, v.nz - 1, v.ov, omp) : 0.0;
+    const double zb = (k >= 1) ? omm * gen::interp_z(v, s.phi, i, j, k, 0, v.nz - 1, v.ov, omm) : 0.0;
+    const double R = -(ax / v.dx + ay / v.dy + (zt - zb)) / v.hc[a];
+    if (diffuse) s.R[a] = R;
+    else s.Qout[a] = s.Qn[a] + s.dts * R;
+  });
+  if (!diffuse) return;
+  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
+    const size_t a = IX(s.v, i, j, k);
+    s.Gx[a] = gx_at(s, i, j, k);
+    s.Gy[a] = gy_at(s, i, j, k);
+  });
+  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
+    const View &v = s.v;
+    const size_t a = IX(v, i, j, k), ip = IX(v, i + 1, j, k), jp = IX(v, i, j + 1, k);
+    // contravariant vertical flux through w-face kk (zero on the lids)
+    auto gz = [&](int kk) -> double {
+      if (kk < 1 || kk > v.nz - 1) return 0.0;
+      const size_t f = IX(v, i, j, kk), b = IX(v, i, j, kk - 1);
+      const double fz = -0.5 * (s.K[b] + s.K[f]) * ((s.phi[f] - s.phi[b]) / v.hw[f]);
+      const double gxb = 0.25 * (s.Gx[b] + s.Gx[IX(v, i + 1, j, kk - 1)] + s.Gx[f] + s.Gx[IX(v, i + 1, j, kk)]);
+      const double gyb = 0.25 * (s.Gy[b] + s.Gy[IX(v, i, j + 1, kk - 1)] + s.Gy[f] + s.Gy[IX(v, i, j + 1, kk)]);
+      return fz - v.sxw[f] * gxb - v.syw[f] * gyb;
+    };
+    const double div = ((v.hx[ip] * s.Gx[ip] - v.hx[a] * s.Gx[a]) / v.dx + (v.hy[jp] * s.Gy[jp] - v.hy[a] * s.Gy[a]) / v.dy +
+                        (gz(k + 1) - gz(k))) / v.hc[a];
+    s.Qout[a] = s.Qn[a] + s.dts * (s.R[a] - div);
+  });
+}
+
+// first use: the scalar, its two stage buffers, the three momentum sums and two work arrays
+bool ensure_scalar(erf_ctx *c) {
+  if (c->sc_Q) return true;
+  double **arr[] = {&c->sc_Q, &c->sc_Qt, &c->sc_Qnew, &c->sc_sum[0], &c->sc_sum[1], &c->sc_sum[2], &c->sc_phi, &c->sc_R};
+  for (auto p : arr) {
+    *p = c->alloc(c->NW);
+    if (!*p) return false;
+  }
+  return true;
+}
+
+}  // namespace erfb

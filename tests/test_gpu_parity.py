@@ -428,3 +428,40 @@ def test_terrain_ragged_and_tiny_sizes(torch, erfo, B, kw):
     assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
     gen = _run_gpu(torch, B, case, 2, path=1)
     assert max(field_errors(got, gen)) <= 2 * TOL_1STEP, field_errors(got, gen)
+
+
+# ---------------------------------------------------------------- transported scalar (Eq. 4)
+@pytest.mark.parametrize("cfg,kw", [(1, dict(nx=40, ny=23, nz=19)), (2, dict(nx=38, ny=19, nz=21)),
+                                    (3, dict(nx=46, ny=21, nz=34)), (5, dict(nx=70, ny=11, nz=40)),
+                                    (4, dict(nx=44, ny=36, nz=96))])
+def test_transported_scalar_matches_oracle(torch, erfo, B, cfg, kw):
+    """rho*phi advanced after the substeps of every stage with the stage-time-averaged momenta: two steps against
+    the oracle, the five prognostic fields unchanged by the scalar's presence, and a constant phi staying constant
+    on the device."""
+    case = wl.make_case(cfg, **kw)
+    rho0 = case["state"][0]
+    rng = np.random.default_rng(300 + cfg)
+    q0 = rho0 * (1.0 + 0.3 * rng.random(rho0.shape))
+    o = erfo.Oracle(case)
+    o.set_state(*case["state"])
+    o.set_scalar(q0)
+    for _ in range(2):
+        o.step(case["dt"], case["ns"])
+    ref, qref = o.get_state(), o.get_scalar()
+    o.close()
+    d = B.Dycore(case)
+    d.set_state(*_dev(torch, case["state"]))
+    d.set_scalar(_dev(torch, [q0])[0])
+    for _ in range(2):
+        d.rk3_step(case["dt"], case["ns"])
+    got, qgot = _host(d.get_state()), d.get_scalar().cpu().numpy()
+    d.set_state(*_dev(torch, case["state"]))
+    d.set_scalar(_dev(torch, [2.5 * rho0])[0])
+    for _ in range(2):
+        d.rk3_step(case["dt"], case["ns"])
+    phi = d.get_scalar().cpu().numpy() / _host(d.get_state())[0]
+    d.close()
+    assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
+    assert np.abs(qgot - qref).max() <= 2 * TOL_1STEP * np.abs(qref).max()
+    assert np.abs(qgot - q0).max() > 1e-8 * np.abs(q0).max()
+    assert np.abs(phi - 2.5).max() <= 1e-12
