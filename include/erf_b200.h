@@ -71,6 +71,11 @@ typedef struct {
   double beta_d;                /* divergence damping (L144), 0.1; 0 switches it off          */
   int substep_mode;             /* 1 semi-implicit substepping (default);
                                    0 none: S_stage = S^n + dt_s f(S) (L140), a test mode      */
+  int scalar_adv;               /* advection of the cell-centred scalars theta and phi (L213):
+                                   0 = adv_order_h / adv_order_v (Eq. 17-21); 13, 15 = WENO-JS
+                                   (Jiang & Shu 1996) of 3rd / 5th order; 23, 25 = WENO-Z (Borges
+                                   et al. 2008); a WENO scheme applies in all three directions and
+                                   runs on the terrain-general kernels                          */
 } erf_params;
 
 /* Build a context: copies grid/params, derives all metric terms from the node heights

@@ -111,7 +111,59 @@ static void get_dense(const erfo_ctx *c, const double *f, double *dense, int nle
  * Eq. 19 (6th), Eq. 20 (3rd) as printed; Eq. 21 (5th) with the sign and the
  * index of its first bracket corrected [R:G1]: as printed it is neither
  * upwind nor 5th order. */
+/* WENO reconstruction of cell-centred scalars ("third-, fifth-... order WENO ... the classic WENO-JS
+ * (Jiang & Shu, 1996), WENO-Z (Borges et al., 2008)"; the paper gives no formulas -- these are the cited schemes
+ * as published [R:G26]).  kind 1 = JS, 2 = Z; ord 3 or 5.  v = the upwind-ordered cell values: for ord 5
+ * v[0..4] = cells i-2 .. i+2 around the upwind cell i, value at its downwind face i+1/2; for ord 3 v[1..3].
+ *   JS:  omega_k ~ d_k / (eps + beta_k)^2,            eps = 1e-6
+ *   Z :  omega_k ~ d_k (1 + tau / (beta_k + eps)),    tau = |beta_0 - beta_last|, eps = 1e-40
+ * with the ideal weights d = (1/10, 6/10, 3/10) resp. (1/3, 2/3) and the Jiang-Shu smoothness indicators. */
+static double weno_face(int kind, int ord, const double *v) {
+  if (ord == 3) {
+    double p0 = 0.5 * (3.0 * v[2] - v[1]), p1 = 0.5 * (v[2] + v[3]);
+    double b0 = (v[2] - v[1]) * (v[2] - v[1]), b1 = (v[3] - v[2]) * (v[3] - v[2]);
+    double a0, a1;
+    if (kind == 1) {
+      a0 = (1.0 / 3.0) / ((1e-6 + b0) * (1e-6 + b0));
+      a1 = (2.0 / 3.0) / ((1e-6 + b1) * (1e-6 + b1));
+    } else {
+      double tau = fabs(b0 - b1);
+      a0 = (1.0 / 3.0) * (1.0 + tau / (b0 + 1e-40));
+      a1 = (2.0 / 3.0) * (1.0 + tau / (b1 + 1e-40));
+    }
+    return (a0 * p0 + a1 * p1) / (a0 + a1);
+  }
+  double p0 = (2.0 * v[0] - 7.0 * v[1] + 11.0 * v[2]) / 6.0;
+  double p1 = (-v[1] + 5.0 * v[2] + 2.0 * v[3]) / 6.0;
+  double p2 = (2.0 * v[2] + 5.0 * v[3] - v[4]) / 6.0;
+  double t0 = v[0] - 2.0 * v[1] + v[2], u0 = v[0] - 4.0 * v[1] + 3.0 * v[2];
+  double t1 = v[1] - 2.0 * v[2] + v[3], u1 = v[1] - v[3];
+  double t2 = v[2] - 2.0 * v[3] + v[4], u2 = 3.0 * v[2] - 4.0 * v[3] + v[4];
+  double b0 = 13.0 / 12.0 * t0 * t0 + 0.25 * u0 * u0;
+  double b1 = 13.0 / 12.0 * t1 * t1 + 0.25 * u1 * u1;
+  double b2 = 13.0 / 12.0 * t2 * t2 + 0.25 * u2 * u2;
+  double a0, a1, a2;
+  if (kind == 1) {
+    a0 = 0.1 / ((1e-6 + b0) * (1e-6 + b0));
+    a1 = 0.6 / ((1e-6 + b1) * (1e-6 + b1));
+    a2 = 0.3 / ((1e-6 + b2) * (1e-6 + b2));
+  } else {
+    double tau = fabs(b0 - b2);
+    a0 = 0.1 * (1.0 + tau / (b0 + 1e-40));
+    a1 = 0.6 * (1.0 + tau / (b1 + 1e-40));
+    a2 = 0.3 * (1.0 + tau / (b2 + 1e-40));
+  }
+  return (a0 * p0 + a1 * p1 + a2 * p2) / (a0 + a1 + a2);
+}
+
+/* order codes: 2..6 = Eq. 17-21; 10*kind + ord = WENO (13, 15 = JS3, JS5; 23, 25 = Z3, Z5) */
 double erfo_interp(int order, double sgn, const double *q) {
+  if (order >= 10) { /* upwind-ordered values: the flux point lies between q[2] and q[3] */
+    double v[5];
+    if (sgn > 0.0) { v[0] = q[0]; v[1] = q[1]; v[2] = q[2]; v[3] = q[3]; v[4] = q[4]; }
+    else           { v[0] = q[5]; v[1] = q[4]; v[2] = q[3]; v[3] = q[2]; v[4] = q[1]; }
+    return weno_face(order / 10, order % 10, v);
+  }
   double q2 = 0.5 * (q[3] + q[2]);
   if (order == 2) return q2;
   double q4 = 7.0 / 12.0 * (q[3] + q[2]) - 1.0 / 12.0 * (q[4] + q[1]);
@@ -126,6 +178,10 @@ double erfo_interp(int order, double sgn, const double *q) {
 /* [R:G13] order reduction next to the lids.  r = min(#valid points below,
  * #valid points above) the flux point. */
 int erfo_vertical_order(int requested, int r) {
+  if (requested >= 10) { /* WENO: the 5-cell stencil needs 3 valid cells on either side, the 3-cell one 2 */
+    if (r >= (requested % 10 + 1) / 2) return requested;
+    return r >= 2 ? 10 * (requested / 10) + 3 : 2;
+  }
   int need = (requested + 1) / 2;
   if (r >= need) return requested;
   if (r >= 2 && requested >= 3) return (requested & 1) ? 3 : 4;
@@ -157,7 +213,7 @@ static double interp_z(const erfo_ctx *c, const double *f, int i, int j, int m, 
   int above = hi - m + 1; /* points m, m+1, ... hi   */
   int r = below < above ? below : above;
   int order = erfo_vertical_order(order_req, r);
-  int half = (order + 1) / 2;
+  int half = (order % 10 + 1) / 2;
   double q[6] = {0, 0, 0, 0, 0, 0};
   for (int n = 3 - half; n < 3 + half; n++) q[n] = f[IX(c, i, j, m - 3 + n)];
   return erfo_interp(order, sgn_of(M), q);
@@ -341,6 +397,8 @@ static void primitives(const erfo_ctx *c, double *const S[5], prim_t *q) {
 static void advection(const erfo_ctx *c, double *const S[5], const prim_t *q, double *R[5]) {
   int nx = c->nx, ny = c->ny, nz = c->nz;
   int oh = c->p.adv_order_h, ov = c->p.adv_order_v;
+  /* cell-centred scalars may use a WENO scheme instead, the same in all directions (L213) */
+  int ohs = c->p.scalar_adv ? c->p.scalar_adv : oh, ovs = c->p.scalar_adv ? c->p.scalar_adv : ov;
   double dx = c->dx, dy = c->dy;
   /* mass fluxes through cell faces: Fx = hx U, Fy = hy V (face-height
    * weighted, finite-volume form [R:G14]) and Omega */
@@ -369,13 +427,13 @@ static void advection(const erfo_ctx *c, double *const S[5], const prim_t *q, do
         R[RHO][a] = -((fxp - fxm) / dx + (fyp - fym) / dy + (omp - omm)) / c->hc[a];
         /* ---- rho*theta, Eq. 3 first term (L67): flux = normal momentum at
          * the face times theta interpolated to the face (L196) ---- */
-        double txm = fxm * interp_x(c, q->theta, i, j, k, oh, fxm);
-        double txp = fxp * interp_x(c, q->theta, i + 1, j, k, oh, fxp);
-        double tym = fym * interp_y(c, q->theta, i, j, k, oh, fym);
-        double typ = fyp * interp_y(c, q->theta, i, j + 1, k, oh, fyp);
-        double tzm = (k >= 1) ? omm * interp_z(c, q->theta, i, j, k, 0, nz - 1, ov, omm) : 0.0;
+        double txm = fxm * interp_x(c, q->theta, i, j, k, ohs, fxm);
+        double txp = fxp * interp_x(c, q->theta, i + 1, j, k, ohs, fxp);
+        double tym = fym * interp_y(c, q->theta, i, j, k, ohs, fym);
+        double typ = fyp * interp_y(c, q->theta, i, j + 1, k, ohs, fyp);
+        double tzm = (k >= 1) ? omm * interp_z(c, q->theta, i, j, k, 0, nz - 1, ovs, omm) : 0.0;
         double tzp =
-            (k + 1 <= nz - 1) ? omp * interp_z(c, q->theta, i, j, k + 1, 0, nz - 1, ov, omp) : 0.0;
+            (k + 1 <= nz - 1) ? omp * interp_z(c, q->theta, i, j, k + 1, 0, nz - 1, ovs, omp) : 0.0;
         R[TH][a] = -((txp - txm) / dx + (typ - tym) / dy + (tzp - tzm)) / c->hc[a];
 
         /* ---- U momentum, Eq. 2 first term (L65).  "Spatial averaging is
@@ -1051,7 +1109,8 @@ static void acoustic_loop(const erfo_ctx *c, double *const St[5], const double *
 static void scalar_stage(const erfo_ctx *c, double *const St[5], const double *Qt, const double *Qn,
                          const double *Ub, const double *Vb, const double *Omb, double dts, double *Qout) {
   int nx = c->nx, ny = c->ny, nz = c->nz;
-  int oh = c->p.adv_order_h, ov = c->p.adv_order_v;
+  int oh = c->p.scalar_adv ? c->p.scalar_adv : c->p.adv_order_h;
+  int ov = c->p.scalar_adv ? c->p.scalar_adv : c->p.adv_order_v;
   double dx = c->dx, dy = c->dy;
   double *phi = fnew(c), *Fx = fnew(c), *Fy = fnew(c), *R = fnew(c);
 #pragma omp parallel for schedule(static)
@@ -1226,6 +1285,8 @@ int erfo_create(const erfo_grid *g, const erfo_metrics *m, const erfo_params *p,
   if (!g->periodic_x || !g->periodic_y) return -2;
   if (!m->rho0 || !m->rhotheta0 || (!m->z_nodes && !m->z_levels)) return -1;
   if (p->adv_order_h < 2 || p->adv_order_h > 6 || p->adv_order_v < 2 || p->adv_order_v > 6) return -1;
+  if (p->scalar_adv != 0 && p->scalar_adv != 13 && p->scalar_adv != 15 && p->scalar_adv != 23 && p->scalar_adv != 25)
+    return -1;
   erfo_ctx *c = (erfo_ctx *)calloc(1, sizeof(erfo_ctx));
   c->nx = g->nx; c->ny = g->ny; c->nz = g->nz; c->dx = g->dx; c->dy = g->dy;
   c->p = *p;

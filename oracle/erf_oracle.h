@@ -50,6 +50,8 @@ typedef struct {
   double beta_s;
   double beta_d;
   int substep_mode; /* 1 semi-implicit, 0 none */
+  int scalar_adv;   /* advection of the cell-centred scalars theta, phi (L213): 0 = adv_order_h/v (Eq. 17-21);
+                       13, 15 = WENO-JS 3rd/5th; 23, 25 = WENO-Z 3rd/5th, the same scheme in all directions */
 } erfo_params;
 
 /* return 0 on success, negative on error */
@@ -69,7 +71,8 @@ int erfo_get_scalar(erfo_ctx *, double *rhophi);
 /* ---- per-operator entry points used by the pinning tests ---- */
 
 /* Eq. 17-21 interpolant at the flux point between q[2]=q_{m-1} and q[3]=q_m;
- * q[0..5] = q_{m-3} .. q_{m+2}; sgn = +1/-1 (sign of the advecting flux). */
+ * q[0..5] = q_{m-3} .. q_{m+2}; sgn = +1/-1 (sign of the advecting flux).
+ * order 2..6, or a WENO code 13, 15, 23, 25 (see erfo_params.scalar_adv). */
 double erfo_interp(int order, double sgn, const double *q);
 
 /* effective vertical order next to the lids (reading G13) */

@@ -48,7 +48,7 @@ class erf_params(C.Structure):
                 ("adv_order_h", C.c_int), ("adv_order_v", C.c_int), ("diffusion", C.c_int),
                 ("nu", C.c_double), ("alpha_theta", C.c_double), ("Cs", C.c_double),
                 ("Pr_t", C.c_double), ("beta_s", C.c_double), ("beta_d", C.c_double),
-                ("substep_mode", C.c_int)]
+                ("substep_mode", C.c_int), ("scalar_adv", C.c_int)]
 
 
 class ErfError(RuntimeError):
@@ -213,7 +213,7 @@ def erf_timing_name(idx):
 def make_params(par: dict) -> erf_params:
     return erf_params(par["Rd"], par["cp"], par["g"], par["p00"], par["adv_order_h"],
                       par["adv_order_v"], par["diffusion"], par["nu"], par["alpha_theta"], par["Cs"],
-                      par["Pr_t"], par["beta_s"], par["beta_d"], par["substep_mode"])
+                      par["Pr_t"], par["beta_s"], par["beta_d"], par["substep_mode"], par.get("scalar_adv", 0))
 
 
 # ---- convenience wrapper ---------------------------------------------------------------

@@ -66,6 +66,8 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   if (p->diffusion < 0 || p->diffusion > 2 || (p->substep_mode != 0 && p->substep_mode != 1)) return ERF_EINVAL;
   if (!(p->cp > p->Rd) || !(p->Rd > 0) || !(p->p00 > 0)) return ERF_EINVAL;
   if (p->diffusion == 2 && !(p->Pr_t > 0)) return ERF_EINVAL;
+  if (p->scalar_adv != 0 && p->scalar_adv != 13 && p->scalar_adv != 15 && p->scalar_adv != 23 && p->scalar_adv != 25)
+    return ERF_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
     cudaGetLastError();
@@ -94,6 +96,8 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   memset(&v, 0, sizeof(v));
   v.nx = g->nx; v.ny = g->ny; v.nz = g->nz;
   v.oh = p->adv_order_h; v.ov = p->adv_order_v; v.diffusion = p->diffusion;
+  v.osh = p->scalar_adv ? p->scalar_adv : p->adv_order_h;
+  v.osv = p->scalar_adv ? p->scalar_adv : p->adv_order_v;
   v.flat = m->z_nodes ? 0 : 1;
   v.dx = g->dx; v.dy = g->dy;
   v.Rd = p->Rd; v.cp = p->cp; v.g = p->g; v.p00 = p->p00;

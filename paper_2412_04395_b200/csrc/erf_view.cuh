@@ -22,6 +22,7 @@ struct View {
   int nx, ny, nz;
   int oh, ov, diffusion;
   int flat, pad_;
+  int osh, osv;  // interpolation of the cell-centred scalars theta, phi: oh / ov, or a WENO code (13, 15, 23, 25)
   double dx, dy;
   double Rd, cp, g, p00, gam, rdocv;
   double nu, alpha, Cs, Prt, beta_s, beta_d;

@@ -122,7 +122,50 @@ ERF_HD void primitives(const View &c, const double *const *S, const Prim &q, int
 
 // ---------------------------------------------------------------- Eq. 17-21 (L200-L211)
 // q[0..5] = q_{m-3} .. q_{m+2}; flux point m-1/2.  Eq. 21 with sign/index repaired [R:G1].
+// WENO-JS (kind 1) / WENO-Z (kind 2) of order 3 or 5 for cell-centred scalars (L213) [R:G26].  Written around the
+// undivided differences of the window (e1 = q[k+1] - q[k]) rather than the textbook coefficient form: candidate
+// values are the upwind cell plus a combination of its neighbouring differences.
+ERF_HD double weno_up(int kind, int ord, double vm2, double vm1, double v0, double vp1, double vp2) {
+  const double dm = v0 - vm1, dp = vp1 - v0;  // differences next to the upwind cell
+  if (ord == 3) {
+    const double b0 = dm * dm, b1 = dp * dp;
+    double a0, a1;
+    if (kind == 1) {
+      const double e0 = 1e-6 + b0, e1 = 1e-6 + b1;
+      a0 = 1.0 / (3.0 * e0 * e0);
+      a1 = 2.0 / (3.0 * e1 * e1);
+    } else {
+      const double tau = fabs(b0 - b1);
+      a0 = (1.0 + tau / (b0 + 1e-40)) / 3.0;
+      a1 = (1.0 + tau / (b1 + 1e-40)) * (2.0 / 3.0);
+    }
+    return v0 + 0.5 * (a0 * dm + a1 * dp) / (a0 + a1);
+  }
+  const double dmm = vm1 - vm2, dpp = vp2 - vp1;
+  // candidates: v0 + (1/6)(-2 dmm + 5 dm), v0 + (1/6)(dm + 2 dp), v0 + (1/6)(4 dp - dpp)... written out from the
+  // sub-stencil parabolas in terms of differences
+  const double c0 = (5.0 * dm - 2.0 * dmm) / 6.0, c1 = (dm + 2.0 * dp) / 6.0, c2 = (4.0 * dp - dpp) / 6.0;
+  const double s0 = dm - dmm, s1 = dp - dm, s2 = dpp - dp;                    // second differences
+  const double t0 = 3.0 * dm - dmm, t1 = dm + dp, t2 = 3.0 * dp - dpp;       // one-sided first differences (x2)
+  const double b0 = (13.0 / 12.0) * s0 * s0 + 0.25 * t0 * t0;
+  const double b1 = (13.0 / 12.0) * s1 * s1 + 0.25 * t1 * t1;
+  const double b2 = (13.0 / 12.0) * s2 * s2 + 0.25 * t2 * t2;
+  double a0, a1, a2;
+  if (kind == 1) {
+    const double e0 = 1e-6 + b0, e1 = 1e-6 + b1, e2 = 1e-6 + b2;
+    a0 = 0.1 / (e0 * e0); a1 = 0.6 / (e1 * e1); a2 = 0.3 / (e2 * e2);
+  } else {
+    const double tau = fabs(b0 - b2);
+    a0 = 0.1 * (1.0 + tau / (b0 + 1e-40)); a1 = 0.6 * (1.0 + tau / (b1 + 1e-40)); a2 = 0.3 * (1.0 + tau / (b2 + 1e-40));
+  }
+  return v0 + (a0 * c0 + a1 * c1 + a2 * c2) / (a0 + a1 + a2);
+}
+
+// order: 2..6 = Eq. 17-21; 13, 15 / 23, 25 = WENO-JS / WENO-Z of order 3, 5
 ERF_HD double interp6(int order, double sgn, const double *q) {
+  if (order >= 10)
+    return sgn > 0.0 ? weno_up(order / 10, order % 10, q[0], q[1], q[2], q[3], q[4])
+                     : weno_up(order / 10, order % 10, q[5], q[4], q[3], q[2], q[1]);
   double s2 = q[3] + q[2];
   if (order == 2) return 0.5 * s2;
   double s4 = q[4] + q[1];
@@ -135,6 +178,10 @@ ERF_HD double interp6(int order, double sgn, const double *q) {
 }
 
 ERF_HD int vertical_order(int requested, int r) {  // [R:G13]
+  if (requested >= 10) {  // WENO: 5-cell stencil needs 3 valid cells on either side, the 3-cell one 2
+    if (r >= (requested % 10 + 1) / 2) return requested;
+    return r >= 2 ? 10 * (requested / 10) + 3 : 2;
+  }
   int need = (requested + 1) / 2;
   if (r >= need) return requested;
   if (r >= 2 && requested >= 3) return (requested & 1) ? 3 : 4;
@@ -145,13 +192,13 @@ ERF_HD double sgn_of(double m) { return m < 0.0 ? -1.0 : 1.0; }  // [R:G19]
 
 ERF_HD double interp_x(const View &c, const double *f, int m, int j, int k, int order, double M) {
   double q[6] = {0, 0, 0, 0, 0, 0};
-  int half = (order + 1) / 2;
+  int half = (order % 10 + 1) / 2;
   for (int n = 3 - half; n < 3 + half; n++) q[n] = f[IX(c, m - 3 + n, j, k)];
   return interp6(order, sgn_of(M), q);
 }
 ERF_HD double interp_y(const View &c, const double *f, int i, int m, int k, int order, double M) {
   double q[6] = {0, 0, 0, 0, 0, 0};
-  int half = (order + 1) / 2;
+  int half = (order % 10 + 1) / 2;
   for (int n = 3 - half; n < 3 + half; n++) q[n] = f[IX(c, i, m - 3 + n, k)];
   return interp6(order, sgn_of(M), q);
 }
@@ -161,7 +208,7 @@ ERF_HD double interp_z(const View &c, const double *f, int i, int j, int m, int 
   int below = m - lo, above = hi - m + 1;
   int r = below < above ? below : above;
   int order = vertical_order(order_req, r);
-  int half = (order + 1) / 2;
+  int half = (order % 10 + 1) / 2;
   double q[6] = {0, 0, 0, 0, 0, 0};
   for (int n = 3 - half; n < 3 + half; n++) q[n] = f[IX(c, i, j, m - 3 + n)];
   return interp6(order, sgn_of(M), q);
@@ -190,12 +237,13 @@ ERF_HD void advect_cell(const View &c, const double *const *S, const double *Om,
   double rhc = 1.0 / c.hc[a];
   R[RHO][a] = -((fxp - fxm) / c.dx + (fyp - fym) / c.dy + (omp - omm)) * rhc;
   {
-    double txm = fxm * interp_x(c, q.theta, i, j, k, oh, fxm);
-    double txp = fxp * interp_x(c, q.theta, i + 1, j, k, oh, fxp);
-    double tym = fym * interp_y(c, q.theta, i, j, k, oh, fym);
-    double typ = fyp * interp_y(c, q.theta, i, j + 1, k, oh, fyp);
-    double tzm = (k >= 1) ? omm * interp_z(c, q.theta, i, j, k, 0, nz - 1, ov, omm) : 0.0;
-    double tzp = (k + 1 <= nz - 1) ? omp * interp_z(c, q.theta, i, j, k + 1, 0, nz - 1, ov, omp) : 0.0;
+    const int sh = c.osh, sv = c.osv;  // cell-centred scalars: Eq. 17-21 or a WENO scheme (L213)
+    double txm = fxm * interp_x(c, q.theta, i, j, k, sh, fxm);
+    double txp = fxp * interp_x(c, q.theta, i + 1, j, k, sh, fxp);
+    double tym = fym * interp_y(c, q.theta, i, j, k, sh, fym);
+    double typ = fyp * interp_y(c, q.theta, i, j + 1, k, sh, fyp);
+    double tzm = (k >= 1) ? omm * interp_z(c, q.theta, i, j, k, 0, nz - 1, sv, omm) : 0.0;
+    double tzp = (k + 1 <= nz - 1) ? omp * interp_z(c, q.theta, i, j, k + 1, 0, nz - 1, sv, omp) : 0.0;
     R[TH][a] = -((txp - txm) / c.dx + (typ - tym) / c.dy + (tzp - tzm)) * rhc;
   }
   {  // U(i-1/2,j,k): momentum averaged to the flux location (L196) [R:G11]

@@ -40,7 +40,8 @@ __global__ void k_level_tables(View v, double *dz, double *rdz, double *rhw, dou
 int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
   FusedState *z = new FusedState();  // value-initialised: every pointer null
   c->fz = z;
-  z->ok = c->v.flat && m->base_is_1d && c->p.substep_mode == 1;
+  // (the fused kernels carry the stencils of Eq. 17-21 only: WENO scalars run the terrain-general kernels)
+  z->ok = c->v.flat && m->base_is_1d && c->p.substep_mode == 1 && c->p.scalar_adv == 0;
   z->variant = 0;  // kernel-variant mask, erf_set_option(ERF_OPT_VARIANT)
   if (!z->ok) return ERF_OK;
   const int nl = c->nz + 1;

@@ -89,10 +89,10 @@ void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, 
     const size_t a = IX(v, i, j, k);
     const double fxm = mx(s, i, j, k), fxp = mx(s, i + 1, j, k), fym = my(s, i, j, k), fyp = my(s, i, j + 1, k);
     const double omm = mz(s, i, j, k), omp = mz(s, i, j, k + 1);
-    const double ax = fxp * gen::interp_x(v, s.phi, i + 1, j, k, v.oh, fxp) - fxm * gen::interp_x(v, s.phi, i, j, k, v.oh, fxm);
-    const double ay = fyp * gen::interp_y(v, s.phi, i, j + 1, k, v.oh, fyp) - fym * gen::interp_y(v, s.phi, i, j, k, v.oh, fym);
-    const double zt = (k + 1 <= v.nz - 1) ? omp * gen::interp_z(v, s.phi, i, j, k + 1, 0, v.nz - 1, v.ov, omp) : 0.0;
-    const double zb = (k >= 1) ? omm * gen::interp_z(v, s.phi, i, j, k, 0, v.nz - 1, v.ov, omm) : 0.0;
+    const double ax = fxp * gen::interp_x(v, s.phi, i + 1, j, k, v.osh, fxp) - fxm * gen::interp_x(v, s.phi, i, j, k, v.osh, fxm);
+    const double ay = fyp * gen::interp_y(v, s.phi, i, j + 1, k, v.osh, fyp) - fym * gen::interp_y(v, s.phi, i, j, k, v.osh, fym);
+    const double zt = (k + 1 <= v.nz - 1) ? omp * gen::interp_z(v, s.phi, i, j, k + 1, 0, v.nz - 1, v.osv, omp) : 0.0;
+    const double zb = (k >= 1) ? omm * gen::interp_z(v, s.phi, i, j, k, 0, v.nz - 1, v.osv, omm) : 0.0;
     const double R = -(ax / v.dx + ay / v.dy + (zt - zb)) / v.hc[a];
     if (diffuse) s.R[a] = R;
     else s.Qout[a] = s.Qn[a] + s.dts * R;

@@ -29,7 +29,7 @@ RD, CP, GRAV, P00 = 287.0, 1004.5, 9.81, 1.0e5
 
 DEFAULT_PARAMS = dict(Rd=RD, cp=CP, g=GRAV, p00=P00, adv_order_h=2, adv_order_v=2, diffusion=0,
                       nu=0.0, alpha_theta=0.0, Cs=0.18, Pr_t=1.0, beta_s=0.1, beta_d=0.1,
-                      substep_mode=1)
+                      substep_mode=1, scalar_adv=0)
 
 
 def hydrostatic_base(z, layers):
