@@ -46,11 +46,11 @@ def test_struct_layouts_match_header():
     assert [f[0] for f in B.erf_grid._fields_] == ["nx", "ny", "nz", "dx", "dy", "periodic_x", "periodic_y"]
     assert C.sizeof(B.erf_grid) == 40
     assert C.sizeof(B.erf_metrics) == 40
-    assert C.sizeof(B.erf_params) == 104  # 4 doubles, 3 ints padded to 16, 6 doubles, 1 int padded to 8
+    assert C.sizeof(B.erf_params) == 104  # 4 doubles, 3 ints padded to 16, 6 doubles, 2 ints
     hdr = open(os.path.join(ROOT, "include", "erf_b200.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
     body = hdr[hdr.index("typedef struct {", hdr.index("erf_metrics;")):hdr.index("} erf_params;")]
-    order = re.findall(r"\b(Rd|cp|g|p00|adv_order_h|adv_order_v|diffusion|nu|alpha_theta|Cs|Pr_t|beta_s|beta_d|substep_mode)\b[,;]", body)
+    order = re.findall(r"\b(Rd|cp|g|p00|adv_order_h|adv_order_v|diffusion|nu|alpha_theta|Cs|Pr_t|beta_s|beta_d|substep_mode|scalar_adv)\b[,;]", body)
     assert order == [f[0] for f in B.erf_params._fields_]
 
 
