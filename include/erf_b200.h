@@ -151,12 +151,11 @@ int erf_set_path(erf_ctx *ctx, int path);
  *                    stream launches.  Meant for grids so small that a step is launch-bound. */
 #define ERF_OPT_VARIANT 1
 #define ERF_OPT_GRAPH 2
-#define ERF_VARIANT_ZC_WIDE 16          /* z-chunked substep kernel: 32-column CTAs            */
-#define ERF_VARIANT_FORCE_ZC 32         /* z-chunked substep kernel on every flat grid         */
 #define ERF_VARIANT_ADV_SPLIT_MASK 192  /* legacy advection: 64 one, 128 two, 192 four launches */
 #define ERF_VARIANT_DIFF_SPLIT 1024     /* momentum and scalar diffusion in separate launches  */
 #define ERF_VARIANT_FORCE_COLUMN 4096   /* thread-per-column substep kernel on every flat grid */
 #define ERF_VARIANT_SPLIT_SLOW_RHS 8192 /* round-1 slow RHS: k_prim_flat + per-field advection */
+#define ERF_VARIANT_FORCE_TILE 16384    /* column-tile substep kernel on every flat grid       */
 int erf_set_option(erf_ctx *ctx, int key, long long value);
 
 /* Number of kernels launched by this context so far (for bench.py's gpu_launches). */

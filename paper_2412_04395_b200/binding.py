@@ -21,8 +21,8 @@ ERF_OK, ERF_EINVAL, ERF_EUNSUPPORTED, ERF_ENOMEM, ERF_ECUDA = 0, -1, -2, -3, -4
 ERF_PATH_AUTO, ERF_PATH_GENERAL = 0, 1
 # erf_set_option keys and ERF_OPT_VARIANT bits (include/erf_b200.h, diagnostics block)
 ERF_OPT_VARIANT, ERF_OPT_GRAPH = 1, 2
-ERF_VARIANT_ZC_WIDE, ERF_VARIANT_FORCE_ZC, ERF_VARIANT_DIFF_SPLIT = 16, 32, 1024
-ERF_VARIANT_FORCE_COLUMN, ERF_VARIANT_SPLIT_SLOW_RHS = 4096, 8192
+ERF_VARIANT_DIFF_SPLIT = 1024
+ERF_VARIANT_FORCE_COLUMN, ERF_VARIANT_SPLIT_SLOW_RHS, ERF_VARIANT_FORCE_TILE = 4096, 8192, 16384
 
 EXPORTS = ["erf_create", "erf_set_state", "erf_rk3_step", "erf_get_state", "erf_destroy",
            "erf_strerror", "erf_set_scalar", "erf_get_scalar", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_set_option", "erf_launch_count",

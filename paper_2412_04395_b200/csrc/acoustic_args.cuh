@@ -1,5 +1,5 @@
-// acoustic_args.cuh -- the argument block shared by the two flat-grid acoustic-substep kernels
-// (k_fused_acoustic.cu: thread per column; k_acoustic_zc.cu: z-chunked) and their common driver.
+// acoustic_args.cuh -- the argument block shared by the flat-grid acoustic-substep kernels (k_acoustic_tile.cu:
+// column tiles with on-chip scratch; k_fused_acoustic.cu: thread per column) and their common driver.
 #pragma once
 #include "fused.cuh"
 
@@ -9,7 +9,7 @@ namespace erfb {
 enum { MODE_FIRST = 1, MODE_LAST = 2, MODE_ZERO = 4 };
 
 struct AcArgs {
-  int nx, ny, nz, M, ZC;
+  int nx, ny, nz;
   int write_cp;  // thread-per-column kernel: store c' (stage constant, so only the first substep of a stage does)
   double dtau, rdx, rdy, b1, b2, beta_d, g, gR;
   const double *Pu, *Pv, *Pw, *Pr, *Pt, *Ptp;  // S'' in: U'', V'', W'', rho'', Theta'' and Theta''_prev
@@ -22,7 +22,7 @@ struct AcArgs {
 };
 
 void launch_acoustic_flat_one(const AcArgs &p, int mode, cudaStream_t st);  // k_fused_acoustic.cu
-bool acoustic_zc_selected(const erf_ctx *c);                                // k_acoustic_zc.cu
-void launch_acoustic_zc_one(const erf_ctx *c, AcArgs &p, int mode, cudaStream_t st);
+bool acoustic_tile_selected(const erf_ctx *c);                              // k_acoustic_tile.cu
+void launch_acoustic_tile_one(const AcArgs &p, int mode, cudaStream_t st);
 
 }  // namespace erfb

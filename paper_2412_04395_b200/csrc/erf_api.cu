@@ -215,8 +215,8 @@ static void drain_timing(erf_ctx *c) {
 extern "C" int erf_set_option(erf_ctx *c, int key, long long value) {
   if (!c) return ERF_EINVAL;
   if (key == ERF_OPT_VARIANT) {
-    const long long known = ERF_VARIANT_ZC_WIDE | ERF_VARIANT_FORCE_ZC | ERF_VARIANT_ADV_SPLIT_MASK |
-                            ERF_VARIANT_DIFF_SPLIT | ERF_VARIANT_FORCE_COLUMN | ERF_VARIANT_SPLIT_SLOW_RHS;
+    const long long known = ERF_VARIANT_ADV_SPLIT_MASK | ERF_VARIANT_DIFF_SPLIT | ERF_VARIANT_FORCE_COLUMN |
+                            ERF_VARIANT_SPLIT_SLOW_RHS | ERF_VARIANT_FORCE_TILE;
     if (value < 0 || (value & ~known)) return ERF_EINVAL;
     if (!c->fz) return ERF_OK;
     if ((value & ERF_VARIANT_SPLIT_SLOW_RHS) && fused_available(c) && !ensure_prim(c, false)) return c->status;

@@ -150,6 +150,10 @@ void general_stage_init(erf_ctx *c, cudaStream_t st);    // P = S - St
 void general_stage_finish(erf_ctx *c, cudaStream_t st);  // St += P, lids
 void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st);
 
+// k_terrain_slow.cu: the advective tendencies of all five fields in one kernel (Eq. 17-21 stencils only)
+bool terrain_advection_available(const erf_ctx *c);
+void launch_terrain_advection(erf_ctx *c, const F5 &S, cudaStream_t st);
+
 // k_scalar.cu: Eq. 4 after the substeps of a stage, with the time-averaged momenta (L138)
 bool ensure_scalar(erf_ctx *c);
 void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, double *Qout, int nsub, double dts,

@@ -125,9 +125,9 @@ void fused_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st) { launch_slow_flat
 static void acoustic_substeps(erf_ctx *c, double dtau, int n, int stage, cudaStream_t st) {
   FusedState *z = c->fz;
   if (n <= 0) return;
-  const bool zc = acoustic_zc_selected(c);
+  const bool tile = acoustic_tile_selected(c);
   AcArgs p;
-  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.M = 0; p.ZC = 0;
+  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
   p.dtau = dtau; p.rdx = 1.0 / c->v.dx; p.rdy = 1.0 / c->v.dy;
   p.b1 = 0.5 * (1.0 - c->v.beta_s); p.b2 = 0.5 * (1.0 + c->v.beta_s);  // L589
   p.beta_d = c->v.beta_d; p.g = c->v.g; p.gR = c->v.gam * c->v.Rd;
@@ -176,7 +176,7 @@ static void acoustic_substeps(erf_ctx *c, double dtau, int n, int stage, cudaStr
     // still holds the stage state that is added at the end (in-place LAST): then the consumed S'' buffers
     if (last && !first) { p.kW = c->P.f[WW]; p.kR = c->P.f[RHO]; p.kT = fr[nfree - 1]; }
     else { p.kW = p.oW; p.kR = p.oR; p.kT = p.oT; }
-    if (zc) launch_acoustic_zc_one(c, p, mode, st);
+    if (tile) launch_acoustic_tile_one(p, mode, st);
     else launch_acoustic_flat_one(p, mode, st);
     c->launches++;
     if (swap_uv) {

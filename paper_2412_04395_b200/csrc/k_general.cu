@@ -105,8 +105,12 @@ void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st) {
   launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) {
     Om[IX(v, i, j, k)] = gen::omega_at(v, Sv.f[UU], Sv.f[VV], Sv.f[WW], i, j, k);
   });
-  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::advect_cell(v, Sv.f, Om, q, R.f, i, j, k); });
-  launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::advect_wface(v, Sv.f, Om, q, R.f, i, j, k); });
+  if (c->path == ERF_PATH_AUTO && terrain_advection_available(c)) {
+    launch_terrain_advection(c, S, st);  // all five advective tendencies in one kernel (k_terrain_slow.cu)
+  } else {
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::advect_cell(v, Sv.f, Om, q, R.f, i, j, k); });
+    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::advect_wface(v, Sv.f, Om, q, R.f, i, j, k); });
+  }
   if (c->p.diffusion != 0) {
     if (!ensure_diff(c)) return;
     gen::Diff d = c->diff;

@@ -187,7 +187,7 @@ def test_config2_full_size_full_step_count(torch, erfo_mt, B):
 def test_full_step_count_on_128_column_crop(torch, erfo_mt, B, cfg, kw):
     """the configuration's own step count (100 / 50 / 20) on a periodic 128 x 128-column crop: four
     CTAs of the tile kernels in x and sixteen in y.  On the flat configurations the thread-per-column substep kernel
-    is forced: it is the one that runs at full size (the library would pick the z-chunked kernel for a grid of
+    is forced: it is the one that runs at full size (the library would pick the column-tile kernel for a grid of
     this few columns)."""
     case = wl.make_case(cfg, **kw)
     steps = case["steps"]
@@ -213,16 +213,18 @@ def test_full_step_count_on_crop(torch, erfo, B, cfg, kw, steps):
     assert max(field_errors(got, ref)) <= min(tol, TOL_100STEP), field_errors(got, ref)
 
 
+@pytest.mark.parametrize("variant", [4096, 16384])
 @pytest.mark.parametrize("cfg,kw,steps", [
     (3, dict(nx=32, ny=24, nz=128), 100),
     (5, dict(nx=32, ny=32, nz=128), 20),
 ])
-def test_full_step_count_on_crop_thread_per_column_kernel(torch, erfo, B, cfg, kw, steps):
-    """The crops above are small enough for the library to pick the z-chunked substep kernel; the kernel that runs
-    at full size (thread per column) gets the same long runs here."""
+def test_full_step_count_on_crop_large_grid_kernels(torch, erfo, B, cfg, kw, steps, variant):
+    """The crops above are small enough for the library to pick the column-tile substep kernel (16384); the kernel
+    that runs at full size (thread per column, 4096) gets the same long runs here, and so does the tile kernel,
+    explicitly."""
     case = wl.make_case(cfg, **kw)
     ref = _run_oracle(erfo, case, steps)
-    got = _run_gpu(torch, B, case, steps, variant=B.ERF_VARIANT_FORCE_COLUMN)
+    got = _run_gpu(torch, B, case, steps, variant=variant)
     tol = TOL_1STEP * steps if steps < 100 else TOL_100STEP
     assert max(field_errors(got, ref)) <= min(tol, TOL_100STEP), field_errors(got, ref)
 
@@ -354,10 +356,11 @@ def test_uses_the_caller_stream(torch, erfo, B):
 
 
 @pytest.mark.parametrize("cfg,kw", [(1, dict(nx=40, ny=23, nz=19)), (3, dict(nx=45, ny=20, nz=34)),
-                                    (5, dict(nx=70, ny=11, nz=40)), (5, dict(nx=33, ny=9, nz=128))])
-@pytest.mark.parametrize("variant", [32, 4096])
+                                    (5, dict(nx=70, ny=11, nz=40)), (5, dict(nx=33, ny=9, nz=128)),
+                                    (2, dict(nx=31, ny=3, nz=5)), (3, dict(nx=64, ny=2, nz=9))])
+@pytest.mark.parametrize("variant", [4096, 16384])
 def test_both_substep_kernels(torch, erfo, B, cfg, kw, variant):
-    """The library picks the substep kernel by grid size (z-chunked partitioned solve, k_acoustic_zc.cu, on
+    """The library picks the substep kernel by grid size (column tiles with on-chip scratch, k_acoustic_tile.cu, on
     grids with few columns; thread per column, k_fused_acoustic.cu, otherwise).  Force each in turn on the same
     small cases: n substeps through erf_acoustic and two full RK3 steps (stage combine folded in)."""
     case = wl.make_case(cfg, **kw)
