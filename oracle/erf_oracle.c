@@ -41,6 +41,7 @@ enum { RHO = 0, UU = 1, VV = 2, WW = 3, TH = 4 };
 
 struct erfo_ctx {
   int nx, ny, nz;
+  int perx, pery; /* lateral boundary per direction: 1 periodic, 0 open */
   double dx, dy;
   erfo_params p;
   double gam, cv, rdocv; /* gamma = cp/(cp-Rd) (L82); cv = cp-Rd; Rd/cv */
@@ -75,14 +76,22 @@ static int wrapi(int a, int n) {
   return r < 0 ? r + n : r;
 }
 
-/* periodic lateral boundary: ghost = image of the interior */
-static void fill_periodic(const erfo_ctx *c, double *f) {
+static int clampi(int a, int n) { return a < 0 ? 0 : (a >= n ? n - 1 : a); }
+
+/* lateral boundary ("periodic, inflow, outflow, or open"), one choice per direction:
+ * periodic: ghost = image of the interior; open: ghost = the nearest interior value (zero normal gradient) for
+ * EVERY field, including the normal momentum, whose first face beyond the last stored one (U at i = nx, V at
+ * j = ny) is such a ghost [R:G27] */
+static void fill_lateral(const erfo_ctx *c, double *f) {
 #pragma omp parallel for schedule(static)
   for (int k = 0; k <= c->nz; k++)
     for (int j = -NG; j < c->ny + NG; j++)
       for (int i = -NG; i < c->nx + NG; i++)
-        if (i < 0 || i >= c->nx || j < 0 || j >= c->ny)
-          f[IX(c, i, j, k)] = f[IX(c, wrapi(i, c->nx), wrapi(j, c->ny), k)];
+        if (i < 0 || i >= c->nx || j < 0 || j >= c->ny) {
+          int is = c->perx ? wrapi(i, c->nx) : clampi(i, c->nx);
+          int js = c->pery ? wrapi(j, c->ny) : clampi(j, c->ny);
+          f[IX(c, i, j, k)] = f[IX(c, is, js, k)];
+        }
 }
 
 static void put_dense(const erfo_ctx *c, double *f, const double *dense, int nlev) {
@@ -91,7 +100,7 @@ static void put_dense(const erfo_ctx *c, double *f, const double *dense, int nle
     for (int j = 0; j < c->ny; j++)
       for (int i = 0; i < c->nx; i++)
         f[IX(c, i, j, k)] = dense[((size_t)k * c->ny + j) * c->nx + i];
-  fill_periodic(c, f);
+  fill_lateral(c, f);
 }
 
 static void get_dense(const erfo_ctx *c, const double *f, double *dense, int nlev) {
@@ -256,9 +265,9 @@ static void build_geometry(erfo_ctx *c, const double *zn) {
             0.25 * (ZN(i, j, k) + ZN(i + 1, j, k) + ZN(i, j + 1, k) + ZN(i + 1, j + 1, k));
       }
 #undef ZN
-  fill_periodic(c, c->zxf);
-  fill_periodic(c, c->zyf);
-  fill_periodic(c, c->zw);
+  fill_lateral(c, c->zxf);
+  fill_lateral(c, c->zyf);
+  fill_lateral(c, c->zw);
 #pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
@@ -268,16 +277,16 @@ static void build_geometry(erfo_ctx *c, const double *zn) {
         c->hc[IX(c, i, j, k)] = c->zw[IX(c, i, j, k + 1)] - c->zw[IX(c, i, j, k)];
         c->zc[IX(c, i, j, k)] = 0.5 * (c->zw[IX(c, i, j, k)] + c->zw[IX(c, i, j, k + 1)]);
       }
-  fill_periodic(c, c->hx);
-  fill_periodic(c, c->hy);
-  fill_periodic(c, c->hc);
-  fill_periodic(c, c->zc);
+  fill_lateral(c, c->hx);
+  fill_lateral(c, c->hy);
+  fill_lateral(c, c->hc);
+  fill_lateral(c, c->zc);
 #pragma omp parallel for schedule(static)
   for (int k = 1; k < nz; k++)
     for (int j = 0; j < ny; j++)
       for (int i = 0; i < nx; i++)
         c->hw[IX(c, i, j, k)] = c->zc[IX(c, i, j, k)] - c->zc[IX(c, i, j, k - 1)];
-  fill_periodic(c, c->hw);
+  fill_lateral(c, c->hw);
 #pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
@@ -287,10 +296,10 @@ static void build_geometry(erfo_ctx *c, const double *zn) {
         c->sxu[IX(c, i, j, k)] = (c->zc[IX(c, i, j, k)] - c->zc[IX(c, i - 1, j, k)]) / c->dx;
         c->syv[IX(c, i, j, k)] = (c->zc[IX(c, i, j, k)] - c->zc[IX(c, i, j - 1, k)]) / c->dy;
       }
-  fill_periodic(c, c->hu);
-  fill_periodic(c, c->hv);
-  fill_periodic(c, c->sxu);
-  fill_periodic(c, c->syv);
+  fill_lateral(c, c->hu);
+  fill_lateral(c, c->hv);
+  fill_lateral(c, c->sxu);
+  fill_lateral(c, c->syv);
 #pragma omp parallel for schedule(static)
   for (int k = 0; k <= nz; k++)
     for (int j = 0; j < ny; j++)
@@ -298,8 +307,8 @@ static void build_geometry(erfo_ctx *c, const double *zn) {
         c->sxw[IX(c, i, j, k)] = (c->zxf[IX(c, i + 1, j, k)] - c->zxf[IX(c, i, j, k)]) / c->dx;
         c->syw[IX(c, i, j, k)] = (c->zyf[IX(c, i, j + 1, k)] - c->zyf[IX(c, i, j, k)]) / c->dy;
       }
-  fill_periodic(c, c->sxw);
-  fill_periodic(c, c->syw);
+  fill_lateral(c, c->sxw);
+  fill_lateral(c, c->syw);
 }
 
 /* ------------------------------------------------------------------ */
@@ -320,7 +329,7 @@ static void impose_lids(const erfo_ctx *c, const double *U, const double *V, dou
           c->sxw[IX(c, i, j, nz)] * 0.5 * (U[IX(c, i, j, nz - 1)] + U[IX(c, i + 1, j, nz - 1)]) +
           c->syw[IX(c, i, j, nz)] * 0.5 * (V[IX(c, i, j, nz - 1)] + V[IX(c, i, j + 1, nz - 1)]);
     }
-  fill_periodic(c, W);
+  fill_lateral(c, W);
 }
 
 /* contravariant vertical mass flux, PAPER.md L196 ("rho*Omega ... normal to
@@ -343,7 +352,7 @@ static void contravariant_flux(const erfo_ctx *c, const double *U, const double 
         }
         Om[IX(c, i, j, k)] = om;
       }
-  fill_periodic(c, Om);
+  fill_lateral(c, Om);
 }
 
 /* ------------------------------------------------------------------ */
@@ -382,12 +391,12 @@ static void primitives(const erfo_ctx *c, double *const S[5], prim_t *q) {
         else rw = 0.5 * (S[RHO][IX(c, i, j, k - 1)] + S[RHO][a]);
         q->w[a] = S[WW][a] / rw;
       }
-  fill_periodic(c, q->theta);
-  fill_periodic(c, q->pp);
-  fill_periodic(c, q->pi);
-  fill_periodic(c, q->u);
-  fill_periodic(c, q->v);
-  fill_periodic(c, q->w);
+  fill_lateral(c, q->theta);
+  fill_lateral(c, q->pp);
+  fill_lateral(c, q->pi);
+  fill_lateral(c, q->u);
+  fill_lateral(c, q->v);
+  fill_lateral(c, q->w);
 }
 
 /* ------------------------------------------------------------------ */
@@ -411,8 +420,8 @@ static void advection(const erfo_ctx *c, double *const S[5], const prim_t *q, do
         Fx[a] = c->hx[a] * S[UU][a];
         Fy[a] = c->hy[a] * S[VV][a];
       }
-  fill_periodic(c, Fx);
-  fill_periodic(c, Fy);
+  fill_lateral(c, Fx);
+  fill_lateral(c, Fy);
   contravariant_flux(c, S[UU], S[VV], S[WW], Om);
 
 #pragma omp parallel for schedule(static)
@@ -550,8 +559,8 @@ static void strain_and_viscosity(const erfo_ctx *c, double *const S[5], const pr
         d->qu[a] = (q->u[a] - q->u[b]) / hwx;
         d->qv[a] = (q->v[a] - q->v[b]) / hwy;
       }
-  fill_periodic(c, d->qu);
-  fill_periodic(c, d->qv);
+  fill_lateral(c, d->qu);
+  fill_lateral(c, d->qv);
   /* S33 first: it is also the vertical quotient of w at centres */
 #pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
@@ -560,7 +569,7 @@ static void strain_and_viscosity(const erfo_ctx *c, double *const S[5], const pr
         size_t a = IX(c, i, j, k);
         d->S33[a] = (q->w[IX(c, i, j, k + 1)] - q->w[a]) / c->hc[a];
       }
-  fill_periodic(c, d->S33);
+  fill_lateral(c, d->S33);
 #pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
@@ -617,11 +626,11 @@ static void strain_and_viscosity(const erfo_ctx *c, double *const S[5], const pr
           d->S23[a] = 0.5 * (d->qv[a] + dwdy);
         }
       }
-  fill_periodic(c, d->S11);
-  fill_periodic(c, d->S22);
-  fill_periodic(c, d->S12);
-  fill_periodic(c, d->S13);
-  fill_periodic(c, d->S23);
+  fill_lateral(c, d->S11);
+  fill_lateral(c, d->S22);
+  fill_lateral(c, d->S12);
+  fill_lateral(c, d->S13);
+  fill_lateral(c, d->S23);
   /* viscosity mu = mu_m + mu_t (L100) and scalar diffusivity K = rho*alpha */
 #pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
@@ -650,8 +659,8 @@ static void strain_and_viscosity(const erfo_ctx *c, double *const S[5], const pr
         d->mu[a] = mu;
         d->K[a] = K;
       }
-  fill_periodic(c, d->mu);
-  fill_periodic(c, d->K);
+  fill_lateral(c, d->mu);
+  fill_lateral(c, d->K);
 }
 
 static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, double *R[5]) {
@@ -689,8 +698,8 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
           t23[a] = -2.0 * mu23 * d.S23[a];
         } /* k = 0 and k = nz stay 0: free slip */
       }
-  fill_periodic(c, t11); fill_periodic(c, t22); fill_periodic(c, t33);
-  fill_periodic(c, t12); fill_periodic(c, t13); fill_periodic(c, t23);
+  fill_lateral(c, t11); fill_lateral(c, t22); fill_lateral(c, t33);
+  fill_lateral(c, t12); fill_lateral(c, t13); fill_lateral(c, t23);
 
   /* vertical two-point quotients of the stresses (for the chain rule) and of theta */
   double *q11 = fnew(c), *q22 = fnew(c), *q12 = fnew(c), *q13 = fnew(c), *q23 = fnew(c);
@@ -702,7 +711,7 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
       for (int i = 0; i < nx; i++)
         ze12[IX(c, i, j, k)] = 0.25 * (c->zc[IX(c, i - 1, j - 1, k)] + c->zc[IX(c, i, j - 1, k)] +
                                        c->zc[IX(c, i - 1, j, k)] + c->zc[IX(c, i, j, k)]);
-  fill_periodic(c, ze12);
+  fill_lateral(c, ze12);
 #pragma omp parallel for schedule(static)
   for (int k = 1; k < nz; k++)
     for (int j = 0; j < ny; j++)
@@ -726,8 +735,8 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
         q13[a] = (t13[t] - t13[a]) / (ze13t - ze13a);
         q23[a] = (t23[t] - t23[a]) / (ze23t - ze23a);
       }
-  fill_periodic(c, q11); fill_periodic(c, q22); fill_periodic(c, q12);
-  fill_periodic(c, q13); fill_periodic(c, q23); fill_periodic(c, qth);
+  fill_lateral(c, q11); fill_lateral(c, q22); fill_lateral(c, q12);
+  fill_lateral(c, q13); fill_lateral(c, q23); fill_lateral(c, qth);
 
   /* ---- momentum: R -= div tau (non-conservative chain-rule form over terrain) ---- */
 #pragma omp parallel for schedule(static)
@@ -791,8 +800,8 @@ static void diffusion(const erfo_ctx *c, double *const S[5], const prim_t *q, do
         Fx[a] = -Kx * dthx;
         Fy[a] = -Ky * dthy;
       }
-  fill_periodic(c, Fx);
-  fill_periodic(c, Fy);
+  fill_lateral(c, Fx);
+  fill_lateral(c, Fy);
 #pragma omp parallel for schedule(static)
   for (int k = 1; k < nz; k++)
     for (int j = 0; j < ny; j++)
@@ -867,6 +876,42 @@ static void pressure_buoyancy(const erfo_ctx *c, double *const S[5], const prim_
       }
 }
 
+/* Rayleigh damping layer ("Rayleigh damping and sponge layer(s)"; Appendix C: "The damping strength,
+ * an inverse timescale, was ramped using a sine-squared function from 0 at the bottom of the damping layer to the
+ * specified value at the top"; Table C1: depth, strength and the damped fields among u, v, w, theta).
+ *   tau(z) = ray_coef * sin^2( (pi/2) (z - z_b) / ray_depth ),  z_b = z_top - ray_depth,  0 below z_b
+ * The paper prints no equation for the tendency; the reading [R:G28] is relaxation of the primitive variable towards a
+ * reference: R_W -= tau W (reference 0), R_U -= tau rho_u (u - u_ref), R_V likewise, R_Theta -= tau rho (theta -
+ * theta0) with theta0 the base state, each tau at the height of its own point.  ray_fields: 1 u, 2 v, 4 w, 8 theta. */
+static double rayleigh_tau(const erfo_ctx *c, double z, double ztop) {
+  double zb = ztop - c->p.ray_depth;
+  if (!(c->p.ray_depth > 0.0) || z <= zb) return 0.0;
+  double s = sin(0.5 * 3.14159265358979323846 * (z - zb) / c->p.ray_depth);
+  return c->p.ray_coef * s * s;
+}
+
+static void rayleigh(const erfo_ctx *c, double *const S[5], double *R[5]) {
+  int nx = c->nx, ny = c->ny, nz = c->nz, f = c->p.ray_fields;
+  if (!f || !(c->p.ray_depth > 0.0)) return;
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < nz; k++)
+    for (int j = 0; j < ny; j++)
+      for (int i = 0; i < nx; i++) {
+        size_t a = IX(c, i, j, k), im = IX(c, i - 1, j, k), jm = IX(c, i, j - 1, k);
+        size_t t = IX(c, i, j, nz), tim = IX(c, i - 1, j, nz), tjm = IX(c, i, j - 1, nz);
+        if (f & 1) {
+          double tau = rayleigh_tau(c, 0.5 * (c->zc[im] + c->zc[a]), 0.5 * (c->zw[tim] + c->zw[t]));
+          R[UU][a] -= tau * (S[UU][a] - 0.5 * (S[RHO][im] + S[RHO][a]) * c->p.ray_uref);
+        }
+        if (f & 2) {
+          double tau = rayleigh_tau(c, 0.5 * (c->zc[jm] + c->zc[a]), 0.5 * (c->zw[tjm] + c->zw[t]));
+          R[VV][a] -= tau * (S[VV][a] - 0.5 * (S[RHO][jm] + S[RHO][a]) * c->p.ray_vref);
+        }
+        if ((f & 4) && k >= 1) R[WW][a] -= rayleigh_tau(c, c->zw[a], c->zw[t]) * S[WW][a];
+        if (f & 8) R[TH][a] -= rayleigh_tau(c, c->zc[a], c->zw[t]) * (S[TH][a] - S[RHO][a] * c->Th0[a] / c->rho0[a]);
+      }
+}
+
 /* f(S): the slow right-hand side of Eq. 1-3.  Also hands back theta^t, pi^t. */
 static void slow_rhs(const erfo_ctx *c, double *const S[5], double *R[5], double *theta_t,
                      double *pi_t) {
@@ -877,7 +922,8 @@ static void slow_rhs(const erfo_ctx *c, double *const S[5], double *R[5], double
   advection(c, S, &q, R);
   if (c->p.diffusion != 0) diffusion(c, S, &q, R);
   pressure_buoyancy(c, S, &q, R);
-  for (int m = 0; m < 5; m++) fill_periodic(c, R[m]);
+  rayleigh(c, S, R);
+  for (int m = 0; m < 5; m++) fill_lateral(c, R[m]);
   if (theta_t) memcpy(theta_t, q.theta, c->n * sizeof(double));
   if (pi_t) memcpy(pi_t, q.pi, c->n * sizeof(double));
   free(q.theta); free(q.pp); free(q.pi); free(q.u); free(q.v); free(q.w);
@@ -947,7 +993,7 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
         Thd[a] = Tpp[a] + c->p.beta_d * (Tpp[a] - ac->Th_prev[a]);
         ac->Th_prev[a] = Tpp[a];
       }
-  fill_periodic(c, Thd);
+  fill_lateral(c, Thd);
 
   /* 2. horizontal momenta, explicit (L585 rows 1-2); pi^t averaged to the face */
 #pragma omp parallel for schedule(static)
@@ -960,8 +1006,8 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
         Upp[a] += dtau * (-gR * piu * grad_x(c, Thd, i, j, k) + ac->R[UU][a]);
         Vpp[a] += dtau * (-gR * piv * grad_y(c, Thd, i, j, k) + ac->R[VV][a]);
       }
-  fill_periodic(c, Upp);
-  fill_periodic(c, Vpp);
+  fill_lateral(c, Upp);
+  fill_lateral(c, Vpp);
   if (ac->Usum) /* the horizontal momenta that enter this substep's continuity equation (step 4) */
     for (size_t a = 0; a < c->n; a++) {
       ac->Usum[a] += Upp[a];
@@ -1060,10 +1106,10 @@ static void acoustic_substep(const erfo_ctx *c, acoustic_t *ac, double dtau) {
   }
   free(om);
   free(Thd);
-  fill_periodic(c, Wpp);
-  fill_periodic(c, Tpp);
-  fill_periodic(c, rpp);
-  fill_periodic(c, ac->Om);
+  fill_lateral(c, Wpp);
+  fill_lateral(c, Tpp);
+  fill_lateral(c, rpp);
+  fill_lateral(c, ac->Om);
 }
 
 /* run n substeps from S'' (ghosts filled) about stage state St */
@@ -1089,7 +1135,7 @@ static void acoustic_loop(const erfo_ctx *c, double *const St[5], const double *
   if (Mavg) /* sums -> time averages over the stage */
     for (int m = 0; m < 3; m++) {
       for (size_t a = 0; a < c->n; a++) Mavg[m][a] /= (double)n;
-      fill_periodic(c, Mavg[m]);
+      fill_lateral(c, Mavg[m]);
     }
   free(ac.Om);
   free(ac.Th_prev);
@@ -1122,9 +1168,9 @@ static void scalar_stage(const erfo_ctx *c, double *const St[5], const double *Q
         Fx[a] = c->hx[a] * Ub[a];
         Fy[a] = c->hy[a] * Vb[a];
       }
-  fill_periodic(c, phi);
-  fill_periodic(c, Fx);
-  fill_periodic(c, Fy);
+  fill_lateral(c, phi);
+  fill_lateral(c, Fx);
+  fill_lateral(c, Fy);
 #pragma omp parallel for schedule(static)
   for (int k = 0; k < nz; k++)
     for (int j = 0; j < ny; j++)
@@ -1159,7 +1205,7 @@ static void scalar_stage(const erfo_ctx *c, double *const St[5], const double *Q
           size_t a = IX(c, i, j, k);
           qph[a] = (phi[a] - phi[IX(c, i, j, k - 1)]) / c->hw[a];
         }
-    fill_periodic(c, qph);
+    fill_lateral(c, qph);
     for (int k = 0; k < nz; k++)
       for (int j = 0; j < ny; j++)
         for (int i = 0; i < nx; i++) {
@@ -1172,8 +1218,8 @@ static void scalar_stage(const erfo_ctx *c, double *const St[5], const double *Q
           Gx[a] = -Kx * dpx;
           Gy[a] = -Ky * dpy;
         }
-    fill_periodic(c, Gx);
-    fill_periodic(c, Gy);
+    fill_lateral(c, Gx);
+    fill_lateral(c, Gy);
     for (int k = 1; k < nz; k++)
       for (int j = 0; j < ny; j++)
         for (int i = 0; i < nx; i++) {
@@ -1202,7 +1248,7 @@ static void scalar_stage(const erfo_ctx *c, double *const St[5], const double *Q
         size_t a = IX(c, i, j, k);
         Qout[a] = Qn[a] + dts * R[a];
       }
-  fill_periodic(c, Qout);
+  fill_lateral(c, Qout);
   free(phi); free(Fx); free(Fy); free(R);
 }
 
@@ -1261,7 +1307,7 @@ int erfo_rk3_step(erfo_ctx *c, double dt, int n_acoustic) {
       for (int m = 0; m < 5; m++) /* L593 */
         for (size_t a = 0; a < c->n; a++) St[m][a] = St[m][a] + P[m][a];
     }
-    for (int m = 0; m < 5; m++) fill_periodic(c, St[m]);
+    for (int m = 0; m < 5; m++) fill_lateral(c, St[m]);
     impose_lids(c, St[UU], St[VV], St[WW]);
   }
   for (int m = 0; m < 5; m++) memcpy(c->S[m], St[m], c->n * sizeof(double));
@@ -1282,13 +1328,13 @@ int erfo_rk3_step(erfo_ctx *c, double dt, int n_acoustic) {
 int erfo_create(const erfo_grid *g, const erfo_metrics *m, const erfo_params *p, erfo_ctx **out) {
   if (!g || !m || !p || !out) return -1;
   if (g->nx < 1 || g->ny < 1 || g->nz < 1 || !(g->dx > 0) || !(g->dy > 0)) return -1;
-  if (!g->periodic_x || !g->periodic_y) return -2;
   if (!m->rho0 || !m->rhotheta0 || (!m->z_nodes && !m->z_levels)) return -1;
   if (p->adv_order_h < 2 || p->adv_order_h > 6 || p->adv_order_v < 2 || p->adv_order_v > 6) return -1;
   if (p->scalar_adv != 0 && p->scalar_adv != 13 && p->scalar_adv != 15 && p->scalar_adv != 23 && p->scalar_adv != 25)
     return -1;
   erfo_ctx *c = (erfo_ctx *)calloc(1, sizeof(erfo_ctx));
   c->nx = g->nx; c->ny = g->ny; c->nz = g->nz; c->dx = g->dx; c->dy = g->dy;
+  c->perx = g->periodic_x != 0; c->pery = g->periodic_y != 0;
   c->p = *p;
   c->cv = p->cp - p->Rd;
   c->gam = p->cp / c->cv;
@@ -1323,8 +1369,8 @@ int erfo_create(const erfo_grid *g, const erfo_metrics *m, const erfo_params *p,
         c->p0[a] = p->p00 * pow(p->Rd * c->Th0[a] / p->p00, c->gam);
         c->pi0[a] = pow(p->Rd * c->Th0[a] / p->p00, c->rdocv);
       }
-  fill_periodic(c, c->rho0); fill_periodic(c, c->Th0);
-  fill_periodic(c, c->p0); fill_periodic(c, c->pi0);
+  fill_lateral(c, c->rho0); fill_lateral(c, c->Th0);
+  fill_lateral(c, c->p0); fill_lateral(c, c->pi0);
   *out = c;
   return 0;
 }

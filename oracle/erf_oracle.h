@@ -30,7 +30,7 @@ typedef struct erfo_ctx erfo_ctx;
 typedef struct {
   int nx, ny, nz;
   double dx, dy;
-  int periodic_x, periodic_y; /* both must be 1 */
+  int periodic_x, periodic_y; /* per direction: 1 periodic (L229); 0 open = zero normal gradient [R:G27] */
 } erfo_grid;
 
 typedef struct {
@@ -52,6 +52,12 @@ typedef struct {
   int substep_mode; /* 1 semi-implicit, 0 none */
   int scalar_adv;   /* advection of the cell-centred scalars theta, phi (L213): 0 = adv_order_h/v (Eq. 17-21);
                        13, 15 = WENO-JS 3rd/5th; 23, 25 = WENO-Z 3rd/5th, the same scheme in all directions */
+  /* Rayleigh damping layer (L219; Appendix C, Table C1): depth below the model top (m; 0 = off), strength at
+   * the top (1/s), sine-squared ramp; damped fields: bit 1 u, 2 v, 4 w, 8 theta; references u_ref, v_ref (m/s),
+   * 0 for w, the base state for theta [R:G28] */
+  double ray_depth, ray_coef;
+  int ray_fields;
+  double ray_uref, ray_vref;
 } erfo_params;
 
 /* return 0 on success, negative on error */

@@ -37,7 +37,9 @@ class Params(C.Structure):
                 ("adv_order_h", C.c_int), ("adv_order_v", C.c_int), ("diffusion", C.c_int),
                 ("nu", C.c_double), ("alpha_theta", C.c_double), ("Cs", C.c_double),
                 ("Pr_t", C.c_double), ("beta_s", C.c_double), ("beta_d", C.c_double),
-                ("substep_mode", C.c_int), ("scalar_adv", C.c_int)]
+                ("substep_mode", C.c_int), ("scalar_adv", C.c_int),
+                ("ray_depth", C.c_double), ("ray_coef", C.c_double), ("ray_fields", C.c_int),
+                ("ray_uref", C.c_double), ("ray_vref", C.c_double)]
 
 
 _SO_OMP = os.path.join(_HERE, "liberf_oracle_omp.so")
@@ -109,7 +111,9 @@ def _c(a):
 def make_params(par: dict) -> Params:
     return Params(par["Rd"], par["cp"], par["g"], par["p00"], par["adv_order_h"],
                   par["adv_order_v"], par["diffusion"], par["nu"], par["alpha_theta"], par["Cs"],
-                  par["Pr_t"], par["beta_s"], par["beta_d"], par["substep_mode"], par.get("scalar_adv", 0))
+                  par["Pr_t"], par["beta_s"], par["beta_d"], par["substep_mode"], par.get("scalar_adv", 0),
+                  par.get("ray_depth", 0.0), par.get("ray_coef", 0.0), par.get("ray_fields", 0),
+                  par.get("ray_uref", 0.0), par.get("ray_vref", 0.0))
 
 
 class Oracle:
@@ -119,7 +123,8 @@ class Oracle:
     def __init__(self, case: dict):
         L = lib()
         self.nx, self.ny, self.nz = case["nx"], case["ny"], case["nz"]
-        g = Grid(self.nx, self.ny, self.nz, case["dx"], case["dy"], 1, 1)
+        g = Grid(self.nx, self.ny, self.nz, case["dx"], case["dy"], int(case.get("periodic_x", 1)),
+                 int(case.get("periodic_y", 1)))
         self._keep = []
         m = Metrics()
         if case.get("z_nodes") is not None:
