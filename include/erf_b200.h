@@ -9,7 +9,8 @@
  *     the perturbation form of Appendix A (L577-L593);
  *   - Arakawa C-grid, terrain-following height coordinate, node heights (L178-L180);
  *   - advective fluxes and the interpolation stencils Eq. 17-21 (L196-L215);
- *   - periodic lateral boundaries (L229), slip-wall lids (L231, Table C1).
+ *   - lateral boundaries periodic or open (L229), slip-wall lids (L231, Table C1), an optional
+ *     Rayleigh damping layer under the model top (L219, L622).
  * Where the paper is silent the discrete reading is "D0", listed in DESIGN.md.
  *
  * Conventions.
@@ -37,7 +38,7 @@ extern "C" {
 
 #define ERF_OK 0
 #define ERF_EINVAL (-1)       /* null pointer, non-positive size, bad order / substep count / dt / option */
-#define ERF_EUNSUPPORTED (-2) /* non-periodic lateral boundary                                   */
+#define ERF_EUNSUPPORTED (-2) /* reserved (no configuration is rejected as unsupported any more)  */
 #define ERF_ENOMEM (-3)       /* host or device allocation failed                                */
 #define ERF_ECUDA (-4)        /* a CUDA runtime call or kernel launch failed (sticky)            */
 
@@ -46,7 +47,9 @@ typedef struct erf_ctx erf_ctx; /* opaque; owns all internal device memory */
 typedef struct {
   int nx, ny, nz;             /* cells */
   double dx, dy;              /* m, uniform (L178) */
-  int periodic_x, periodic_y; /* must both be 1 (L229), else ERF_EUNSUPPORTED */
+  int periodic_x, periodic_y; /* per direction: 1 periodic; 0 open (L229 "periodic, inflow, outflow, or open"):
+                                 every ghost value is the nearest interior value (zero normal gradient,
+                                 DESIGN.md reading G27); open grids run the terrain-general kernels      */
 } erf_grid;
 
 typedef struct {
@@ -76,6 +79,12 @@ typedef struct {
                                    (Jiang & Shu 1996) of 3rd / 5th order; 23, 25 = WENO-Z (Borges
                                    et al. 2008); a WENO scheme applies in all three directions and
                                    runs on the terrain-general kernels                          */
+  double ray_depth, ray_coef;   /* Rayleigh damping layer (L219; Appendix C, Table C1): depth below the
+                                   model top in m (0 = off) and strength at the top in 1/s; the strength
+                                   ramps as sine squared from 0 at the bottom of the layer               */
+  int ray_fields;               /* damped fields: bit 1 u, 2 v, 4 w, 8 theta                             */
+  double ray_uref, ray_vref;    /* m/s: u, v relax towards these; w towards 0, theta towards the base
+                                   state (reading G28)                                        */
 } erf_params;
 
 /* Build a context: copies grid/params, derives all metric terms from the node heights

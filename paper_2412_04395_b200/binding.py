@@ -48,7 +48,9 @@ class erf_params(C.Structure):
                 ("adv_order_h", C.c_int), ("adv_order_v", C.c_int), ("diffusion", C.c_int),
                 ("nu", C.c_double), ("alpha_theta", C.c_double), ("Cs", C.c_double),
                 ("Pr_t", C.c_double), ("beta_s", C.c_double), ("beta_d", C.c_double),
-                ("substep_mode", C.c_int), ("scalar_adv", C.c_int)]
+                ("substep_mode", C.c_int), ("scalar_adv", C.c_int),
+                ("ray_depth", C.c_double), ("ray_coef", C.c_double), ("ray_fields", C.c_int),
+                ("ray_uref", C.c_double), ("ray_vref", C.c_double)]
 
 
 class ErfError(RuntimeError):
@@ -213,7 +215,9 @@ def erf_timing_name(idx):
 def make_params(par: dict) -> erf_params:
     return erf_params(par["Rd"], par["cp"], par["g"], par["p00"], par["adv_order_h"],
                       par["adv_order_v"], par["diffusion"], par["nu"], par["alpha_theta"], par["Cs"],
-                      par["Pr_t"], par["beta_s"], par["beta_d"], par["substep_mode"], par.get("scalar_adv", 0))
+                      par["Pr_t"], par["beta_s"], par["beta_d"], par["substep_mode"], par.get("scalar_adv", 0),
+                      par.get("ray_depth", 0.0), par.get("ray_coef", 0.0), par.get("ray_fields", 0),
+                      par.get("ray_uref", 0.0), par.get("ray_vref", 0.0))
 
 
 # ---- convenience wrapper ---------------------------------------------------------------
@@ -229,7 +233,8 @@ class Dycore:
             raise RuntimeError("no CUDA device: liberf_b200 has no CPU fallback")
         self.device = torch.device(device)
         self.nx, self.ny, self.nz = case["nx"], case["ny"], case["nz"]
-        g = erf_grid(self.nx, self.ny, self.nz, case["dx"], case["dy"], 1, 1)
+        g = erf_grid(self.nx, self.ny, self.nz, case["dx"], case["dy"], int(case.get("periodic_x", 1)),
+                     int(case.get("periodic_y", 1)))
         m = erf_metrics()
         keep = []
 

@@ -37,7 +37,7 @@ extern "C" const char *erf_strerror(int code) {
   switch (code) {
     case ERF_OK: return "ok";
     case ERF_EINVAL: return "invalid argument";
-    case ERF_EUNSUPPORTED: return "unsupported configuration (lateral boundaries must be periodic)";
+    case ERF_EUNSUPPORTED: return "unsupported configuration";
     case ERF_ENOMEM: return "out of memory";
     case ERF_ECUDA: return "CUDA error";
     default: return "unknown error";
@@ -60,7 +60,6 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   if (!g || !m || !p || !out) return ERF_EINVAL;
   *out = nullptr;
   if (g->nx < 1 || g->ny < 1 || g->nz < 1 || !(g->dx > 0) || !(g->dy > 0)) return ERF_EINVAL;
-  if (!g->periodic_x || !g->periodic_y) return ERF_EUNSUPPORTED;
   if (!m->rho0 || !m->rhotheta0 || (!m->z_nodes && !m->z_levels)) return ERF_EINVAL;
   if (p->adv_order_h < 2 || p->adv_order_h > 6 || p->adv_order_v < 2 || p->adv_order_v > 6) return ERF_EINVAL;
   if (p->diffusion < 0 || p->diffusion > 2 || (p->substep_mode != 0 && p->substep_mode != 1)) return ERF_EINVAL;
@@ -68,6 +67,7 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   if (p->diffusion == 2 && !(p->Pr_t > 0)) return ERF_EINVAL;
   if (p->scalar_adv != 0 && p->scalar_adv != 13 && p->scalar_adv != 15 && p->scalar_adv != 23 && p->scalar_adv != 25)
     return ERF_EINVAL;
+  if (p->ray_depth < 0.0 || p->ray_coef < 0.0 || p->ray_fields < 0 || p->ray_fields > 15) return ERF_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
     cudaGetLastError();
@@ -99,6 +99,9 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   v.osh = p->scalar_adv ? p->scalar_adv : p->adv_order_h;
   v.osv = p->scalar_adv ? p->scalar_adv : p->adv_order_v;
   v.flat = m->z_nodes ? 0 : 1;
+  v.perx = g->periodic_x != 0; v.pery = g->periodic_y != 0;
+  v.ray_fields = p->ray_depth > 0.0 && p->ray_coef > 0.0 ? p->ray_fields : 0;
+  v.ray_depth = p->ray_depth; v.ray_coef = p->ray_coef; v.ray_uref = p->ray_uref; v.ray_vref = p->ray_vref;
   v.dx = g->dx; v.dy = g->dy;
   v.Rd = p->Rd; v.cp = p->cp; v.g = p->g; v.p00 = p->p00;
   v.gam = p->cp / (p->cp - p->Rd);    // L82

@@ -3,8 +3,8 @@
 //
 // HBM layout: every 3-D field is dense, x fastest, [nlev][ny][nx] with nlev = nz (cell
 // and horizontal-face fields) or nz+1 (w-face fields); all are allocated with nz+1
-// levels.  There are no ghost cells: the periodic lateral boundary is
-// an index wrap at load time, so no halo-fill pass ever touches HBM.
+// levels.  There are no ghost cells: the lateral boundary is an index wrap (periodic) or an index
+// clamp (open) at load time, so no halo-fill pass ever touches HBM.
 #pragma once
 #include <cstddef>
 
@@ -21,7 +21,10 @@ enum { RHO = 0, UU = 1, VV = 2, WW = 3, TH = 4 };
 struct View {
   int nx, ny, nz;
   int oh, ov, diffusion;
-  int flat, pad_;
+  int flat;
+  int perx, pery;  // lateral boundary per direction: 1 periodic (index wrap), 0 open (index clamp) [R:G27]
+  int ray_fields;  // Rayleigh layer: bit 1 u, 2 v, 4 w, 8 theta (0 = off)
+  double ray_depth, ray_coef, ray_uref, ray_vref;
   int osh, osv;  // interpolation of the cell-centred scalars theta, phi: oh / ov, or a WENO code (13, 15, 23, 25)
   double dx, dy;
   double Rd, cp, g, p00, gam, rdocv;
@@ -51,9 +54,13 @@ ERF_HD int wrapi(int a, int n) {
   return a;
 }
 
-// periodic index into a dense [.][ny][nx] field
+// open boundary: the ghost value is the nearest interior value, i.e. the index is clamped
+ERF_HD int clampi(int a, int n) { return a < 0 ? 0 : (a >= n ? n - 1 : a); }
+ERF_HD int lati(int a, int n, int periodic) { return periodic ? wrapi(a, n) : clampi(a, n); }
+
+// index into a dense [.][ny][nx] field with the lateral boundary condition folded in
 ERF_HD size_t IX(const View &c, int i, int j, int k) {
-  return ((size_t)k * c.ny + wrapi(j, c.ny)) * c.nx + wrapi(i, c.nx);
+  return ((size_t)k * c.ny + lati(j, c.ny, c.pery)) * c.nx + lati(i, c.nx, c.perx);
 }
 
 }  // namespace erfb

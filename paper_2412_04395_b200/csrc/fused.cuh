@@ -25,6 +25,8 @@ struct LevelTables {
   const double *p0;     // [k] base-state pressure (Eq. 7)
   const double *pi0;    // [k] base-state Exner function
   const double *csd2;   // [k] (Cs Delta)^2, Delta = (dx dy dz_k)^(1/3)  [R:G9]
+  const double *tauc;   // [k] Rayleigh damping rate at cell centres (L622) [R:G28]
+  const double *tauw;   // [k] ... and at w-faces
 };
 
 struct FusedState {
@@ -36,6 +38,7 @@ struct FusedState {
   double *cp_scr;     // Thomas c' of the thread-per-column substep kernel (stage constant)
   double *mu, *Kd;    // dynamic viscosity and scalar diffusivity at cell centres (diffusion != 0)
   std::map<const void *, CUtensorMap> tmaps;  // TMA tensor maps of the state buffers (k_slow_adv.cu)
+  int ray_k0;         // first level with a non-zero Rayleigh rate (nz: none)
   int variant;        // ERF_VARIANT_* mask (erf_set_option, diagnostics block of erf_b200.h); 0 = defaults
 };
 

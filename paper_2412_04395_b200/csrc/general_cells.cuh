@@ -553,6 +553,35 @@ ERF_HD void pgbuoy_cell(const View &c, const double *const *S, const Prim &q, do
   }
 }
 
+// ---------------------------------------------------------------- Rayleigh damping layer (L219, L622) [R:G28]
+// tau(z) = ray_coef sin^2((pi/2)(z - z_b)/ray_depth) above z_b = z_top - ray_depth (L622: sine-squared ramp from 0 at
+// the bottom of the layer to the stated inverse time scale at the top)
+ERF_HD double rayleigh_tau(double depth, double coef, double z, double ztop) {
+  const double zb = ztop - depth;
+  if (z <= zb) return 0.0;
+  const double s = sin(0.5 * 3.14159265358979323846 * (z - zb) / depth);
+  return coef * s * s;
+}
+
+// relaxation of the masked primitives towards their references (u_ref, v_ref, 0, theta0), k < nz
+ERF_HD void rayleigh_cell(const View &c, const double *const *S, double *const *R, int i, int j, int k) {
+  const int nz = c.nz, f = c.ray_fields;
+  const size_t a = IX(c, i, j, k), t = IX(c, i, j, nz);
+  if (f & 1) {
+    const size_t im = IX(c, i - 1, j, k), tim = IX(c, i - 1, j, nz);
+    const double tau = rayleigh_tau(c.ray_depth, c.ray_coef, 0.5 * (c.zc[im] + c.zc[a]), 0.5 * (c.zw[tim] + c.zw[t]));
+    R[UU][a] -= tau * (S[UU][a] - 0.5 * (S[RHO][im] + S[RHO][a]) * c.ray_uref);
+  }
+  if (f & 2) {
+    const size_t jm = IX(c, i, j - 1, k), tjm = IX(c, i, j - 1, nz);
+    const double tau = rayleigh_tau(c.ray_depth, c.ray_coef, 0.5 * (c.zc[jm] + c.zc[a]), 0.5 * (c.zw[tjm] + c.zw[t]));
+    R[VV][a] -= tau * (S[VV][a] - 0.5 * (S[RHO][jm] + S[RHO][a]) * c.ray_vref);
+  }
+  if ((f & 4) && k >= 1) R[WW][a] -= rayleigh_tau(c.ray_depth, c.ray_coef, c.zw[a], c.zw[t]) * S[WW][a];
+  if (f & 8)
+    R[TH][a] -= rayleigh_tau(c.ray_depth, c.ray_coef, c.zc[a], c.zw[t]) * (S[TH][a] - S[RHO][a] * c.Th0[a] / c.rho0[a]);
+}
+
 // ---------------------------------------------------------------- acoustic substeps (S5)
 struct Acou {
   const double *theta_t, *pi_t, *Th_t;  // stage constants

@@ -165,7 +165,9 @@ __global__ void __launch_bounds__(128, 2) k_acoustic_terrain(const AcTerr p) {
 }
 
 // ------------------------------------------------------------------ driver
-bool terrain_acoustic_available(const erf_ctx *c) { return !c->v.flat && c->p.substep_mode == 1; }
+bool terrain_acoustic_available(const erf_ctx *c) {
+  return !c->v.flat && c->p.substep_mode == 1 && c->v.perx && c->v.pery;  // the kernel wraps its neighbour indices
+}
 
 // n substeps of size dtau about the stage state St (theta_t, pi_t, R, P set by the caller): general_acoustic with
 // its three heavy passes per substep fused into k_acoustic_terrain

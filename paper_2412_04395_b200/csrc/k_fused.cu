@@ -8,10 +8,17 @@ namespace erfb {
 
 // per-level tables from column (0,0) of the 3-D geometry / base-state fields
 __global__ void k_level_tables(View v, double *dz, double *rdz, double *rhw, double *tabB, double *rho0,
-                               double *Th0, double *rTh0, double *p0, double *pi0, double *csd2) {
+                               double *Th0, double *rTh0, double *p0, double *pi0, double *csd2, double *tauc,
+                               double *tauw) {
   int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k > v.nz) return;
   size_t a = (size_t)k * v.ny * v.nx;
+  {  // Rayleigh damping rates (L622) [R:G28]
+    const double ztop = v.zw[(size_t)v.nz * v.ny * v.nx];
+    const bool on = v.ray_fields != 0;
+    tauw[k] = on ? gen::rayleigh_tau(v.ray_depth, v.ray_coef, v.zw[a], ztop) : 0.0;
+    tauc[k] = on && k < v.nz ? gen::rayleigh_tau(v.ray_depth, v.ray_coef, v.zc[a], ztop) : 0.0;
+  }
   if (k < v.nz) {
     dz[k] = v.hc[a];
     rdz[k] = 1.0 / v.hc[a];
@@ -41,7 +48,8 @@ int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
   FusedState *z = new FusedState();  // value-initialised: every pointer null
   c->fz = z;
   // (the fused kernels carry the stencils of Eq. 17-21 only: WENO scalars run the terrain-general kernels)
-  z->ok = c->v.flat && m->base_is_1d && c->p.substep_mode == 1 && c->p.scalar_adv == 0;
+  // ... and periodic boundaries only: open grids run the terrain-general kernels, whose index helper clamps
+  z->ok = c->v.flat && m->base_is_1d && c->p.substep_mode == 1 && c->p.scalar_adv == 0 && c->v.perx && c->v.pery;
   z->variant = 0;  // kernel-variant mask, erf_set_option(ERF_OPT_VARIANT)
   if (!z->ok) return ERF_OK;
   const int nl = c->nz + 1;
@@ -58,7 +66,7 @@ int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
   double *zxf = col[0], *zyf = col[1], *zw = col[2], *hx = col[3], *hy = col[4], *hc = col[5], *zc = col[6];
   double *hw = col[7], *hu = col[8], *hv = col[9], *sxu = col[10], *syv = col[11], *sxw = col[12], *syw = col[13];
   double *rho0 = col[14], *Th0 = col[15], *p0 = col[16], *pi0 = col[17];
-  vc.hc = hc; vc.hw = hw; vc.rho0 = rho0; vc.Th0 = Th0; vc.p0 = p0; vc.pi0 = pi0;
+  vc.hc = hc; vc.hw = hw; vc.rho0 = rho0; vc.Th0 = Th0; vc.p0 = p0; vc.pi0 = pi0; vc.zw = zw; vc.zc = zc;
   gen::NodeH Z;
   Z.zn = nullptr; Z.zl = c->zl_dev; Z.nx = 1; Z.ny = 1;
   const double *r0in = c->base1d_r0, *t0in = c->base1d_T0;
@@ -74,14 +82,23 @@ int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
     gen::geo_derived(vv, zxf, zyf, hc, zc, hw, hu, hv, sxu, syv, sxw, syw, i, j, k);
   });
   column(nz, [=] __device__(int i, int j, int k) { gen::base_state(vv, r0in, t0in, 1, rho0, Th0, p0, pi0, i, j, k); });
-  double *t[10];
+  double *t[12];
   for (auto &p : t) {
     p = c->alloc(nl);
     if (!p) return c->status;
   }
-  k_level_tables<<<(nl + 127) / 128, 128, 0, st>>>(vc, t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7], t[8], t[9]);
+  k_level_tables<<<(nl + 127) / 128, 128, 0, st>>>(vc, t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7], t[8], t[9], t[10],
+                                                   t[11]);
   c->launches++;
-  z->tab = LevelTables{t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7], t[8], t[9]};
+  z->tab = LevelTables{t[0], t[1], t[2], t[3], t[4], t[5], t[6], t[7], t[8], t[9], t[10], t[11]};
+  // the layer's first level, from the host copy of the level heights (the rates themselves come from the device)
+  z->ray_k0 = c->nz;
+  if (c->v.ray_fields && m->z_levels) {
+    const double zb = m->z_levels[c->nz] - c->v.ray_depth;
+    int k0 = 0;
+    while (k0 < c->nz && m->z_levels[k0 + 1] <= zb) k0++;  // cell k0 is the first whose top face lies above z_b
+    z->ray_k0 = k0;
+  }
   double **arr[] = {&z->iT, &z->U2, &z->V2, &z->Thd[0], &z->Thd[1], &z->cp_scr};
   for (auto p : arr) {
     *p = c->alloc(c->NW);

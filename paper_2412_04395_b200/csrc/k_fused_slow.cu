@@ -45,6 +45,21 @@ __global__ void __launch_bounds__(256) k_prim_flat(const SlowFlat p) {
   }
 }
 
+// Rayleigh damping layer (L219, L622) [R:G28] on the levels k0 .. nz-1 that the layer reaches: relaxation of the masked
+// primitives towards (u_ref, v_ref, 0, theta0); the rates are per-level tables on a flat grid
+__global__ void __launch_bounds__(256) k_rayleigh_flat(const SlowFlat p, const double *__restrict__ tauc,
+                                                       const double *__restrict__ tauw, int k0, int fields,
+                                                       double uref, double vref) {
+  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k = k0 + blockIdx.z;
+  if (i >= p.nx || j >= p.ny) return;
+  const size_t kk = (size_t)k * p.nx * p.ny, a = kk + (size_t)j * p.nx + i;
+  const double tc = tauc[k], rc = p.rho[a];
+  if (fields & 1) p.RU[a] -= tc * (p.U[a] - 0.5 * (p.rho[kk + (size_t)j * p.nx + (i == 0 ? p.nx - 1 : i - 1)] + rc) * uref);
+  if (fields & 2) p.RV[a] -= tc * (p.V[a] - 0.5 * (p.rho[kk + (size_t)(j == 0 ? p.ny - 1 : j - 1) * p.nx + i] + rc) * vref);
+  if ((fields & 4) && k >= 1) p.RW[a] -= tauw[k] * p.W[a];
+  if (fields & 8) p.RTh[a] -= tc * (p.Th[a] - rc * p.Th0[k] / p.rho0[k]);
+}
+
 void launch_slow_flat(erf_ctx *c, const F5 &S, cudaStream_t st) {
   Timed t(c, T_SLOW_FUSED, st);
   FusedState *z = c->fz;
@@ -73,6 +88,12 @@ void launch_slow_flat(erf_ctx *c, const F5 &S, cudaStream_t st) {
   if (c->p.diffusion != 0) {
     launch_visc_tiled(c, p, st);
     launch_diff_tiled(c, p, st);
+  }
+  if (z->ray_k0 < c->nz) {
+    dim3 block(32, 8), grid((c->nx + 31) / 32, (c->ny + 7) / 8, c->nz - z->ray_k0);
+    k_rayleigh_flat<<<grid, block, 0, st>>>(p, z->tab.tauc, z->tab.tauw, z->ray_k0, c->v.ray_fields, c->v.ray_uref,
+                                            c->v.ray_vref);
+    c->launches++;
   }
 }
 

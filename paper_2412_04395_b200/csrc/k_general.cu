@@ -125,6 +125,8 @@ void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st) {
     launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass8(v, d, R.f, i, j, k); });
   }
   launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::pgbuoy_cell(v, Sv.f, q, R.f, i, j, k); });
+  if (v.ray_fields)  // Rayleigh damping layer (L219, L622)
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::rayleigh_cell(v, Sv.f, R.f, i, j, k); });
   // stage constants for the substeps: theta^t, pi^t
   cudaMemcpyAsync(c->theta_t, q.theta, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
   cudaMemcpyAsync(c->pi_t, q.pi, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);

@@ -6,8 +6,8 @@
 //   theta, u, v, w (L196) and the stencils of Eq. 17-21 (L198-L211) in the branch-free form
 //   flux = M q_even - |M| q_odd [R:G1], vertical order reduced next to the lids [R:G13].
 //
-// One thread per cell, one level per blockIdx.z (so the vertical order is uniform over a CTA).  The seven periodic
-// column offsets in x and in y are wrapped once per thread; every stencil value is then one load at
+// One thread per cell, one level per blockIdx.z (so the vertical order is uniform over a CTA).  The seven column
+// offsets in x and in y are wrapped (periodic) or clamped (open boundary) once per thread; every stencil value is then one load at
 // level base + row offset + column offset, served by L1/L2 (neighbouring threads share all but one point).  This
 // replaces the two terrain-general advection passes (general_cells.cuh advect_cell / advect_wface: a run-time
 // order, a wrapped index per stencil point), which stay as the ERF_PATH_GENERAL cross-check.
@@ -22,7 +22,7 @@ struct Args {
   const double *th, *u, *v, *w;          // advected primitives
   const double *hx, *hy, *hc, *hu, *hv, *hw;
   double *Rrho, *RU, *RV, *RW, *RTh;
-  int nx, ny, nz, ov;
+  int nx, ny, nz, ov, perx, pery;
   double rdx, rdy;
 };
 
@@ -41,8 +41,8 @@ __global__ void __launch_bounds__(256) k_adv_terrain(const Args p) {
   size_t yo[7];
 #pragma unroll
   for (int n = 0; n < 7; n++) {
-    xo[n] = wrapi(i + n - 3, nx);
-    yo[n] = (size_t)wrapi(j + n - 3, ny) * nx;
+    xo[n] = lati(i + n - 3, nx, p.perx);
+    yo[n] = (size_t)lati(j + n - 3, ny, p.pery) * nx;
   }
   const size_t oc = yo[3] + xo[3], a = kb + oc;
   const bool low = k >= 1, up = k + 1 <= nz - 1;
@@ -148,7 +148,7 @@ void launch_terrain_advection(erf_ctx *c, const F5 &S, cudaStream_t st) {
   p.th = c->prim.theta; p.u = c->prim.u; p.v = c->prim.v; p.w = c->prim.w;
   p.hx = v.hx; p.hy = v.hy; p.hc = v.hc; p.hu = v.hu; p.hv = v.hv; p.hw = v.hw;
   p.Rrho = c->R.f[RHO]; p.RU = c->R.f[UU]; p.RV = c->R.f[VV]; p.RW = c->R.f[WW]; p.RTh = c->R.f[TH];
-  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.ov = v.ov;
+  p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.ov = v.ov; p.perx = v.perx; p.pery = v.pery;
   p.rdx = 1.0 / v.dx; p.rdy = 1.0 / v.dy;
   dim3 block(32, 8), grid((c->nx + 31) / 32, (c->ny + 7) / 8, c->nz);
   switch (v.oh) {

@@ -46,11 +46,11 @@ def test_struct_layouts_match_header():
     assert [f[0] for f in B.erf_grid._fields_] == ["nx", "ny", "nz", "dx", "dy", "periodic_x", "periodic_y"]
     assert C.sizeof(B.erf_grid) == 40
     assert C.sizeof(B.erf_metrics) == 40
-    assert C.sizeof(B.erf_params) == 104  # 4 doubles, 3 ints padded to 16, 6 doubles, 2 ints
+    assert C.sizeof(B.erf_params) == 144  # 4 doubles, 3 ints padded to 16, 6 doubles, 2 ints, 2 doubles, int (padded), 2 doubles
     hdr = open(os.path.join(ROOT, "include", "erf_b200.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
     body = hdr[hdr.index("typedef struct {", hdr.index("erf_metrics;")):hdr.index("} erf_params;")]
-    order = re.findall(r"\b(Rd|cp|g|p00|adv_order_h|adv_order_v|diffusion|nu|alpha_theta|Cs|Pr_t|beta_s|beta_d|substep_mode|scalar_adv)\b[,;]", body)
+    order = re.findall(r"\b(Rd|cp|g|p00|adv_order_h|adv_order_v|diffusion|nu|alpha_theta|Cs|Pr_t|beta_s|beta_d|substep_mode|scalar_adv|ray_depth|ray_coef|ray_fields|ray_uref|ray_vref)\b[,;]", body)
     assert order == [f[0] for f in B.erf_params._fields_]
 
 
@@ -76,8 +76,8 @@ def test_create_validates_before_cuda(lib):
     h = C.c_void_p()
     assert lib.erf_create(None, C.byref(m), C.byref(p), None, C.byref(h)) == B.ERF_EINVAL
     assert lib.erf_create(C.byref(g), C.byref(m), C.byref(p), None, None) == B.ERF_EINVAL
-    g2, *_ = _args(case, periodic=(1, 0))
-    assert lib.erf_create(C.byref(g2), C.byref(m), C.byref(p), None, C.byref(h)) == B.ERF_EUNSUPPORTED
+    bad = dict(case["params"]); bad["ray_fields"] = 16
+    assert lib.erf_create(C.byref(g), C.byref(m), C.byref(B.make_params(bad)), None, C.byref(h)) == B.ERF_EINVAL
     bad = dict(case["params"]); bad["adv_order_h"] = 7
     assert lib.erf_create(C.byref(g), C.byref(m), C.byref(B.make_params(bad)), None, C.byref(h)) == B.ERF_EINVAL
     g3 = B.erf_grid(0, 4, 4, 1.0, 1.0, 1, 1)

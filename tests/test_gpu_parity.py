@@ -498,3 +498,59 @@ def test_weno_scalars_match_oracle(torch, erfo, B, cfg, kw, code):
     # is amplified where beta ~ eps; 1e-10 of the field maximum holds with a wide margin (observed ~1e-13)
     assert max(field_errors(got, ref)) <= 1e-10, field_errors(got, ref)
     assert np.abs(qgot - qref).max() <= 1e-10 * np.abs(qref).max()
+
+
+# ---------------------------------------------------------------- open lateral boundaries (L229) and Rayleigh layer (L219, L622)
+@pytest.mark.parametrize("per", [(0, 1), (1, 0), (0, 0)])
+@pytest.mark.parametrize("cfg,kw", [(2, dict(nx=38, ny=19, nz=21)), (5, dict(nx=70, ny=11, nz=40)),
+                                    (4, dict(nx=44, ny=36, nz=96))])
+def test_open_boundaries_match_oracle(torch, erfo, B, cfg, kw, per):
+    """Open (zero normal gradient) lateral boundaries in x, in y and in both: f(S) of a developed state and two full
+    steps against the oracle, on flat crops and over the hill (the hill sits away from the boundary)."""
+    case = wl.make_case(cfg, **kw)
+    case["periodic_x"], case["periodic_y"] = per
+    st = _run_oracle(erfo, case, 1)
+    o = erfo.Oracle(case)
+    o.set_state(*st)
+    ref_R = o.slow_rhs()
+    o.close()
+    d = B.Dycore(case)
+    d.set_state(*_dev(torch, st))
+    got_R = _host(d.slow_rhs())
+    d.close()
+    for f, (a, b) in enumerate(zip(got_R, ref_R)):
+        assert np.abs(a - b).max() <= TOL_RHS * max(np.abs(b).max(), 1e-300), (f, per)
+    ref = _run_oracle(erfo, case, 2)
+    got = _run_gpu(torch, B, case, 2)
+    assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
+    # the open closure is not the periodic one
+    per_case = dict(case, periodic_x=1, periodic_y=1)
+    assert max(field_errors(_run_gpu(torch, B, per_case, 2), ref)) > 1e-9
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("cfg,kw,mask", [(3, dict(nx=46, ny=21, nz=34), 15), (5, dict(nx=70, ny=11, nz=40), 5),
+                                         (1, dict(nx=40, ny=23, nz=19), 9), (4, dict(nx=44, ny=36, nz=96), 15)])
+def test_rayleigh_layer_matches_oracle(torch, erfo, B, cfg, kw, mask, path):
+    """The Rayleigh damping layer under the model top (sine-squared ramp, masked fields) on the fused flat path, on
+    the general path and over terrain: f(S) and two steps against the oracle; the layer must actually do something."""
+    base = wl.make_case(cfg, **kw)
+    top = base["z_levels"][-1] if base.get("z_nodes") is None else float(base["z_nodes"][-1].max())
+    case = wl.make_case(cfg, params=dict(ray_depth=0.3 * top, ray_coef=0.2, ray_fields=mask, ray_uref=3.0,
+                                         ray_vref=-1.0), **kw)
+    st = _run_oracle(erfo, case, 1)
+    o = erfo.Oracle(case)
+    o.set_state(*st)
+    ref_R = o.slow_rhs()
+    o.close()
+    d = B.Dycore(case)
+    d.set_path(path)
+    d.set_state(*_dev(torch, st))
+    got_R = _host(d.slow_rhs())
+    d.close()
+    for f, (a, b) in enumerate(zip(got_R, ref_R)):
+        assert np.abs(a - b).max() <= TOL_RHS * max(np.abs(b).max(), 1e-300), f
+    ref = _run_oracle(erfo, case, 2)
+    got = _run_gpu(torch, B, case, 2, path)
+    assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
+    assert max(field_errors(_run_gpu(torch, B, base, 2, path), ref)) > 1e-8
