@@ -251,6 +251,8 @@ def run_ours(args):
     dyc = binding.Dycore(case, device=f"cuda:{local}")
     if args.path:
         dyc.set_path(args.path)
+    if args.variant:
+        dyc.set_option(binding.ERF_OPT_VARIANT, args.variant)
     host = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in case["state"]]
     dev = [h.cuda(non_blocking=True) for h in host]
     dyc.set_state(*dev)
@@ -445,7 +447,7 @@ def run_ours(args):
                 "fields fit in L2 (small configuration)",
                 "replicas": world, "device_bytes": dev_bytes, "repeats": max(args.repeats, 1),
                 "ms_per_step_repeats": [r / args.steps for r in reps],
-                "path": "general" if args.path == 1 else "auto"})
+                "path": "general" if args.path == 1 else "auto", "variant": args.variant})
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg, "clocks": clk.summary(),
@@ -473,6 +475,7 @@ def main():
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--path", type=int, default=0, choices=[0, 1], help="0 auto (fused), 1 general kernels")
+    ap.add_argument("--variant", type=int, default=0, help="ERF_VARIANT_* developer mask (include/erf_b200.h), 0 = defaults")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-all-configs", action="store_true", help="skip the configs 1-4 summary of the default run")
     ap.add_argument("--repeats", type=int, default=5, help="timed repeats of the K steps (median reported)")
