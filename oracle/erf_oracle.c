@@ -42,6 +42,7 @@ enum { RHO = 0, UU = 1, VV = 2, WW = 3, TH = 4 };
 struct erfo_ctx {
   int nx, ny, nz;
   int perx, pery; /* lateral boundary per direction: 1 periodic, 0 open */
+  int flat;       /* z_nodes == NULL: level heights depend on k only */
   double dx, dy;
   erfo_params p;
   double gam, cv, rdocv; /* gamma = cp/(cp-Rd) (L82); cv = cp-Rd; Rd/cv */
@@ -59,6 +60,8 @@ struct erfo_ctx {
   double *S[5];
   /* one transported scalar rho*phi (Eq. 4); NULL until erfo_set_scalar */
   double *Q;
+  /* anelastic mode (Sec. 2.2, 3.2): the lagged perturbation pressure p' of the projection; NULL until first used */
+  double *pan;
 };
 
 /* ------------------------------------------------------------------ */
@@ -913,20 +916,28 @@ static void rayleigh(const erfo_ctx *c, double *const S[5], double *R[5]) {
 }
 
 /* f(S): the slow right-hand side of Eq. 1-3.  Also hands back theta^t, pi^t. */
-static void slow_rhs(const erfo_ctx *c, double *const S[5], double *R[5], double *theta_t,
-                     double *pi_t) {
+static void anelastic_pressure_buoyancy(const erfo_ctx *c, const prim_t *q, const double *pan, double *R[5]);
+
+static void slow_rhs_mode(const erfo_ctx *c, double *const S[5], double *R[5], double *theta_t,
+                          double *pi_t, const double *pan) {
   prim_t q;
   q.theta = fnew(c); q.pp = fnew(c); q.pi = fnew(c);
   q.u = fnew(c); q.v = fnew(c); q.w = fnew(c);
   primitives(c, S, &q);
   advection(c, S, &q, R);
   if (c->p.diffusion != 0) diffusion(c, S, &q, R);
-  pressure_buoyancy(c, S, &q, R);
+  if (pan) anelastic_pressure_buoyancy(c, &q, pan, R); /* Sec. 2.2: p' from the projection, B from theta */
+  else pressure_buoyancy(c, S, &q, R);
   rayleigh(c, S, R);
   for (int m = 0; m < 5; m++) fill_lateral(c, R[m]);
   if (theta_t) memcpy(theta_t, q.theta, c->n * sizeof(double));
   if (pi_t) memcpy(pi_t, q.pi, c->n * sizeof(double));
   free(q.theta); free(q.pp); free(q.pi); free(q.u); free(q.v); free(q.w);
+}
+
+static void slow_rhs(const erfo_ctx *c, double *const S[5], double *R[5], double *theta_t,
+                     double *pi_t) {
+  slow_rhs_mode(c, S, R, theta_t, pi_t, NULL);
 }
 
 /* ------------------------------------------------------------------ */
@@ -1322,6 +1333,224 @@ int erfo_rk3_step(erfo_ctx *c, double dt, int n_acoustic) {
 }
 
 /* ------------------------------------------------------------------ */
+/* Anelastic mode (Sec. 2.2 L88-L96 Eq. 8; Sec. 3.2 */
+/* Eq. 14-16).  Flat, laterally periodic grids (stretched levels ok).  */
+/* ------------------------------------------------------------------ */
+
+/* L96: "the buoyancy force B for dry air [is] rho0 (theta - theta0)/theta0 g"; "the pressure perturbation p' that enters
+ * the momentum equation is computed solely from the Poisson equation".  R_U -= Gx(p'), R_V -= Gy(p') with the operators of
+ * S4; at w-faces R_W -= (p'(k) - p'(k-1))/hw(k) and R_W += g * mean of B/g over the two adjacent cells [R:G11]. */
+static void anelastic_pressure_buoyancy(const erfo_ctx *c, const prim_t *q, const double *pan, double *R[5]) {
+  int nx = c->nx, ny = c->ny, nz = c->nz;
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < nz; k++)
+    for (int j = 0; j < ny; j++)
+      for (int i = 0; i < nx; i++) {
+        size_t a = IX(c, i, j, k);
+        R[UU][a] -= grad_x(c, pan, i, j, k);
+        R[VV][a] -= grad_y(c, pan, i, j, k);
+        if (k >= 1) {
+          size_t b = IX(c, i, j, k - 1);
+          double th0a = c->Th0[a] / c->rho0[a], th0b = c->Th0[b] / c->rho0[b];
+          double Ba = c->rho0[a] * (q->theta[a] - th0a) / th0a, Bb = c->rho0[b] * (q->theta[b] - th0b) / th0b;
+          R[WW][a] += -(pan[a] - pan[b]) / c->hw[a] + c->p.g * 0.5 * (Bb + Ba);
+        }
+      }
+}
+
+/* discrete divergence of the momenta at cell centres: D(M) = dU/dx + dV/dy + dW/dz (flat grid: Omega = W, hx = hy = hc) */
+static void divergence(const erfo_ctx *c, const double *U, const double *V, const double *W, double *D) {
+  int nx = c->nx, ny = c->ny, nz = c->nz;
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < nz; k++)
+    for (int j = 0; j < ny; j++)
+      for (int i = 0; i < nx; i++) {
+        size_t a = IX(c, i, j, k);
+        D[a] = (U[IX(c, i + 1, j, k)] - U[a]) / c->dx + (V[IX(c, i, j + 1, k)] - V[a]) / c->dy +
+               (W[IX(c, i, j, k + 1)] - W[a]) / c->hc[a];
+      }
+}
+
+/* Eq. 16: dt div(grad psi) = div(rho0 u**), then rho0 u* = rho0 u** - dt grad psi and p' += psi (L158-L162).
+ * grad psi lives on the faces: (psi(i) - psi(i-1))/dx, (psi(j) - psi(j-1))/dy, (psi(k) - psi(k-1))/hw(k) on interior
+ * w-faces, nothing on the rigid lids (W = 0 there): the discrete Laplacian is div of this grad, symmetric, with the
+ * constants as its null space.  "ERF provides several options for solving the Poisson equation: geometric multigrid,
+ * Fast Fourier Transforms (FFTs) and ..." (L164): here the discrete Fourier transform in the two periodic directions,
+ * written out as its definition, and one tridiagonal system in z per horizontal mode (m, n):
+ *   [lx(m) + ly(n)] P_k + [ (P_{k+1} - P_k)/hw_{k+1} - (P_k - P_{k-1})/hw_k ] / dz_k = Dhat_k / dt,
+ *   lx(m) = -(4/dx^2) sin^2(pi m / nx),  ly(n) = -(4/dy^2) sin^2(pi n / ny);
+ * the singular mode (0, 0) is fixed by psi_hat(k = 0) = 0 [R:G29]. */
+static void project(erfo_ctx *c, double *U, double *V, double *W, double dt) {
+  int nx = c->nx, ny = c->ny, nz = c->nz;
+  const double PI = 3.14159265358979323846;
+  size_t nh = (size_t)nx * ny;
+  double *D = fnew(c);
+  divergence(c, U, V, W, D);
+  /* forward transform: Dhat(m, n, k) = sum_{i,j} D(i, j, k) exp(-2 pi I (m i / nx + n j / ny)) */
+  double *Ar = (double *)malloc(nh * nz * sizeof(double)), *Ai = (double *)malloc(nh * nz * sizeof(double));
+  double *Br = (double *)malloc(nh * nz * sizeof(double)), *Bi = (double *)malloc(nh * nz * sizeof(double));
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < nz; k++) {
+    for (int j = 0; j < ny; j++)
+      for (int m = 0; m < nx; m++) { /* x */
+        double sr = 0.0, si = 0.0;
+        for (int i = 0; i < nx; i++) {
+          double ph = -2.0 * PI * (double)((long long)m * i % nx) / nx;
+          double d = D[IX(c, i, j, k)];
+          sr += d * cos(ph);
+          si += d * sin(ph);
+        }
+        Ar[(size_t)k * nh + (size_t)j * nx + m] = sr;
+        Ai[(size_t)k * nh + (size_t)j * nx + m] = si;
+      }
+    for (int n = 0; n < ny; n++)
+      for (int m = 0; m < nx; m++) { /* y */
+        double sr = 0.0, si = 0.0;
+        for (int j = 0; j < ny; j++) {
+          double ph = -2.0 * PI * (double)((long long)n * j % ny) / ny;
+          double cr = cos(ph), ci = sin(ph);
+          double ar = Ar[(size_t)k * nh + (size_t)j * nx + m], ai = Ai[(size_t)k * nh + (size_t)j * nx + m];
+          sr += ar * cr - ai * ci;
+          si += ar * ci + ai * cr;
+        }
+        Br[(size_t)k * nh + (size_t)n * nx + m] = sr;
+        Bi[(size_t)k * nh + (size_t)n * nx + m] = si;
+      }
+  }
+  /* one real tridiagonal matrix per mode, solved (Thomas) for the real and the imaginary part */
+#pragma omp parallel for schedule(static)
+  for (int n = 0; n < ny; n++)
+    for (int m = 0; m < nx; m++) {
+      double sx = sin(PI * m / nx), sy = sin(PI * n / ny);
+      double lam = -4.0 * sx * sx / (c->dx * c->dx) - 4.0 * sy * sy / (c->dy * c->dy);
+      double *cp = (double *)malloc(nz * sizeof(double));
+      double *dr = (double *)malloc(nz * sizeof(double)), *di = (double *)malloc(nz * sizeof(double));
+      for (int k = 0; k < nz; k++) {
+        size_t a = IX(c, 0, 0, k); /* flat grid: level metrics from column (0, 0) */
+        double dz = c->hc[a];
+        double lo = k >= 1 ? 1.0 / (c->hw[a] * dz) : 0.0;
+        double up = k <= nz - 2 ? 1.0 / (c->hw[IX(c, 0, 0, k + 1)] * dz) : 0.0;
+        double diag = lam - lo - up;
+        size_t q = (size_t)k * nh + (size_t)n * nx + m;
+        double rr = Br[q] / dt, ri = Bi[q] / dt;
+        if (m == 0 && n == 0 && k == 0) { lo = 0.0; up = 0.0; diag = 1.0; rr = 0.0; ri = 0.0; }
+        double den = diag - (k >= 1 ? lo * cp[k - 1] : 0.0);
+        cp[k] = up / den;
+        dr[k] = (rr - (k >= 1 ? lo * dr[k - 1] : 0.0)) / den;
+        di[k] = (ri - (k >= 1 ? lo * di[k - 1] : 0.0)) / den;
+      }
+      for (int k = nz - 1; k >= 0; k--) {
+        size_t q = (size_t)k * nh + (size_t)n * nx + m;
+        double pr = dr[k] - (k <= nz - 2 ? cp[k] * Br[q + nh] : 0.0);
+        double pi = di[k] - (k <= nz - 2 ? cp[k] * Bi[q + nh] : 0.0);
+        Br[q] = pr;
+        Bi[q] = pi;
+      }
+      free(cp); free(dr); free(di);
+    }
+  /* inverse transform (real part; the imaginary part vanishes for a real right-hand side) */
+  double *psi = fnew(c);
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < nz; k++) {
+    for (int j = 0; j < ny; j++)
+      for (int m = 0; m < nx; m++) { /* y */
+        double sr = 0.0, si = 0.0;
+        for (int n = 0; n < ny; n++) {
+          double ph = 2.0 * PI * (double)((long long)n * j % ny) / ny;
+          double cr = cos(ph), ci = sin(ph);
+          double br = Br[(size_t)k * nh + (size_t)n * nx + m], bi = Bi[(size_t)k * nh + (size_t)n * nx + m];
+          sr += br * cr - bi * ci;
+          si += br * ci + bi * cr;
+        }
+        Ar[(size_t)k * nh + (size_t)j * nx + m] = sr;
+        Ai[(size_t)k * nh + (size_t)j * nx + m] = si;
+      }
+    for (int j = 0; j < ny; j++)
+      for (int i = 0; i < nx; i++) { /* x */
+        double sr = 0.0;
+        for (int m = 0; m < nx; m++) {
+          double ph = 2.0 * PI * (double)((long long)m * i % nx) / nx;
+          sr += Ar[(size_t)k * nh + (size_t)j * nx + m] * cos(ph) - Ai[(size_t)k * nh + (size_t)j * nx + m] * sin(ph);
+        }
+        psi[IX(c, i, j, k)] = sr / ((double)nx * ny);
+      }
+  }
+  free(Ar); free(Ai); free(Br); free(Bi);
+  fill_lateral(c, psi);
+  /* correct the momenta, accumulate the pressure */
+#pragma omp parallel for schedule(static)
+  for (int k = 0; k < nz; k++)
+    for (int j = 0; j < ny; j++)
+      for (int i = 0; i < nx; i++) {
+        size_t a = IX(c, i, j, k);
+        U[a] -= dt * (psi[a] - psi[IX(c, i - 1, j, k)]) / c->dx;
+        V[a] -= dt * (psi[a] - psi[IX(c, i, j - 1, k)]) / c->dy;
+        if (k >= 1) W[a] -= dt * (psi[a] - psi[IX(c, i, j, k - 1)]) / c->hw[a];
+        c->pan[a] += psi[a];
+      }
+  fill_lateral(c, U); fill_lateral(c, V); fill_lateral(c, W); fill_lateral(c, c->pan);
+  free(D); free(psi);
+}
+
+static int anelastic_ok(erfo_ctx *c, int flat) {
+  if (!c || !flat || !c->perx || !c->pery) return 0;
+  if (!c->pan) c->pan = fnew(c);
+  return 1;
+}
+
+/* test entry points: project the current momenta with time step dt; the divergence of the current momenta; p' */
+int erfo_project(erfo_ctx *c, double dt) {
+  if (!anelastic_ok(c, c ? c->flat : 0) || !(dt > 0.0)) return -1;
+  project(c, c->S[UU], c->S[VV], c->S[WW], dt);
+  return 0;
+}
+
+int erfo_divergence(erfo_ctx *c, double *D) {
+  if (!c || !D) return -1;
+  double *d = fnew(c);
+  divergence(c, c->S[UU], c->S[VV], c->S[WW], d);
+  get_dense(c, d, D, c->nz);
+  free(d);
+  return 0;
+}
+
+int erfo_get_pprime(erfo_ctx *c, double *pp) {
+  if (!c || !pp || !c->pan) return -1;
+  get_dense(c, c->pan, pp, c->nz);
+  return 0;
+}
+
+/* One RK2 step of the anelastic equations (Eq. 14-15), a projection after each stage (L154-L162):
+ *   S*      = S^n + dt f(S^n),                  projected with dt;
+ *   S^{n+1} = S^n + dt/2 (f(S^n) + f(S*)),      projected with dt ("an analogous procedure", L162).
+ * rho is held at rho0 ("we can replace rho_d by rho_0 ... which makes the continuity equation redundant", L94): the
+ * density of the context's state is overwritten by the base state.  f is f(S) of the compressible core with the
+ * pressure-gradient / buoyancy pair of Sec. 2.2; no acoustic substeps ("with no substepping in each RK stage", L148).
+ * p' accumulates psi after EACH projection, as printed (L160) [R:G29]. */
+int erfo_anelastic_step(erfo_ctx *c, double dt) {
+  if (!anelastic_ok(c, c ? c->flat : 0) || !(dt > 0.0)) return -1;
+  memcpy(c->S[RHO], c->rho0, c->n * sizeof(double));
+  double *St[5], *R1[5], *R2[5];
+  for (int m = 0; m < 5; m++) { St[m] = fnew(c); R1[m] = fnew(c); R2[m] = fnew(c); }
+  slow_rhs_mode(c, c->S, R1, NULL, NULL, c->pan);
+  for (int m = 0; m < 5; m++)
+    for (size_t a = 0; a < c->n; a++) St[m][a] = m == RHO ? c->S[m][a] : c->S[m][a] + dt * R1[m][a];
+  for (int m = 0; m < 5; m++) fill_lateral(c, St[m]);
+  impose_lids(c, St[UU], St[VV], St[WW]);
+  project(c, St[UU], St[VV], St[WW], dt);
+  slow_rhs_mode(c, St, R2, NULL, NULL, c->pan);
+  for (int m = 0; m < 5; m++)
+    for (size_t a = 0; a < c->n; a++)
+      St[m][a] = m == RHO ? c->S[m][a] : c->S[m][a] + 0.5 * dt * (R1[m][a] + R2[m][a]);
+  for (int m = 0; m < 5; m++) fill_lateral(c, St[m]);
+  impose_lids(c, St[UU], St[VV], St[WW]);
+  project(c, St[UU], St[VV], St[WW], dt);
+  for (int m = 0; m < 5; m++) memcpy(c->S[m], St[m], c->n * sizeof(double));
+  for (int m = 0; m < 5; m++) { free(St[m]); free(R1[m]); free(R2[m]); }
+  return 0;
+}
+
+/* ------------------------------------------------------------------ */
 /* context                                                             */
 /* ------------------------------------------------------------------ */
 
@@ -1335,6 +1564,7 @@ int erfo_create(const erfo_grid *g, const erfo_metrics *m, const erfo_params *p,
   erfo_ctx *c = (erfo_ctx *)calloc(1, sizeof(erfo_ctx));
   c->nx = g->nx; c->ny = g->ny; c->nz = g->nz; c->dx = g->dx; c->dy = g->dy;
   c->perx = g->periodic_x != 0; c->pery = g->periodic_y != 0;
+  c->flat = m->z_nodes == NULL;
   c->p = *p;
   c->cv = p->cp - p->Rd;
   c->gam = p->cp / c->cv;
@@ -1382,6 +1612,7 @@ void erfo_destroy(erfo_ctx *c) {
                    c->S[0], c->S[1], c->S[2], c->S[3], c->S[4]};
   for (size_t a = 0; a < sizeof(all) / sizeof(all[0]); a++) free(all[a]);
   free(c->Q);
+  free(c->pan);
   free(c);
 }
 

@@ -74,6 +74,14 @@ void erfo_destroy(erfo_ctx *);
 int erfo_set_scalar(erfo_ctx *, const double *rhophi);
 int erfo_get_scalar(erfo_ctx *, double *rhophi);
 
+/* Anelastic mode (Sec. 2.2 Eq. 8, Sec. 3.2 Eq. 14-16): one RK2 step of size dt with a projection after each
+ * stage; flat, laterally periodic grids only (else -1).  rho of the state is held at the base state rho0; the lagged
+ * perturbation pressure p' (zero at first) lives in the context. */
+int erfo_anelastic_step(erfo_ctx *, double dt);
+int erfo_get_pprime(erfo_ctx *, double *pprime);     /* [nz][ny][nx] */
+int erfo_project(erfo_ctx *, double dt);             /* Eq. 16 applied to the current momenta */
+int erfo_divergence(erfo_ctx *, double *D);          /* dU/dx + dV/dy + dW/dz of the current momenta, [nz][ny][nx] */
+
 /* ---- per-operator entry points used by the pinning tests ---- */
 
 /* Eq. 17-21 interpolant at the flux point between q[2]=q_{m-1} and q[3]=q_m;

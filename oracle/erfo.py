@@ -82,6 +82,10 @@ def lib():
         L.erfo_rk3_step.argtypes = [C.c_void_p, C.c_double, C.c_int]
         L.erfo_set_scalar.argtypes = [C.c_void_p, _dp]
         L.erfo_get_scalar.argtypes = [C.c_void_p, _dp]
+        L.erfo_anelastic_step.argtypes = [C.c_void_p, C.c_double]
+        L.erfo_get_pprime.argtypes = [C.c_void_p, _dp]
+        L.erfo_project.argtypes = [C.c_void_p, C.c_double]
+        L.erfo_divergence.argtypes = [C.c_void_p, _dp]
         L.erfo_destroy.argtypes = [C.c_void_p]
         L.erfo_destroy.restype = None
         L.erfo_interp.argtypes = [C.c_int, C.c_double, _dp]
@@ -195,6 +199,24 @@ class Oracle:
         rc = self._L.erfo_rk3_step(self._h, float(dt), int(n_acoustic))
         if rc != 0:
             raise RuntimeError(f"erfo_rk3_step failed: {rc}")
+
+    def anelastic_step(self, dt):
+        rc = self._L.erfo_anelastic_step(self._h, float(dt))
+        if rc != 0:
+            raise RuntimeError(f"erfo_anelastic_step failed: {rc}")
+
+    def project(self, dt):
+        assert self._L.erfo_project(self._h, float(dt)) == 0
+
+    def divergence(self):
+        out = np.empty(self.shape_c)
+        assert self._L.erfo_divergence(self._h, _p(out)) == 0
+        return out
+
+    def pprime(self):
+        out = np.empty(self.shape_c)
+        assert self._L.erfo_get_pprime(self._h, _p(out)) == 0
+        return out
 
     def slow_rhs(self):
         out = [np.empty(self.shape_c), np.empty(self.shape_c), np.empty(self.shape_c),
