@@ -38,7 +38,7 @@ extern "C" {
 
 #define ERF_OK 0
 #define ERF_EINVAL (-1)       /* null pointer, non-positive size, bad order / substep count / dt / option */
-#define ERF_EUNSUPPORTED (-2) /* reserved (no configuration is rejected as unsupported any more)  */
+#define ERF_EUNSUPPORTED (-2) /* anelastic mode on a terrain or laterally open grid                */
 #define ERF_ENOMEM (-3)       /* host or device allocation failed                                */
 #define ERF_ECUDA (-4)        /* a CUDA runtime call or kernel launch failed (sticky)            */
 
@@ -119,6 +119,19 @@ int erf_get_state(erf_ctx *ctx, double *rho, double *rhou, double *rhov, double 
  * (ERF_PATH_GENERAL) for the whole step.  erf_get_scalar before erf_set_scalar: ERF_EINVAL. */
 int erf_set_scalar(erf_ctx *ctx, const double *rhophi, void *cuda_stream);
 int erf_get_scalar(erf_ctx *ctx, double *rhophi, void *cuda_stream);
+
+/* Anelastic mode (Sec. 2.2 Eq. 8; Sec. 3.2 Eq. 14-16): one RK2 step of size dt of the anelastic
+ * equations, no substepping, with a projection after each of the two stages:  dt div(grad psi) = div(rho0 u**),
+ * rho0 u* = rho0 u** - dt grad psi,  p' += psi.  The buoyancy is rho0 (theta - theta0)/theta0 g and the pressure
+ * gradient uses the lagged p' of the projections only (L96); rho of the state is overwritten by the base state rho0
+ * (L94).  The Poisson equation is solved by a discrete Fourier transform in x and y and a tridiagonal system in z per
+ * mode (reading G29), so the grid must be flat and periodic in x and y: otherwise ERF_EUNSUPPORTED.
+ * Uses the same context, state and parameters as erf_rk3_step; p' starts at zero and lives in the context.
+ * erf_get_pprime: DEVICE [nz][ny][nx]; ERF_EINVAL before the first anelastic call.
+ * erf_project applies the projection alone to the momenta of the current state (tests). */
+int erf_anelastic_step(erf_ctx *ctx, double dt, void *cuda_stream);
+int erf_get_pprime(erf_ctx *ctx, double *pprime, void *cuda_stream);
+int erf_project(erf_ctx *ctx, double dt, void *cuda_stream);
 
 /* Free everything; erf_destroy(NULL) is a no-op. */
 void erf_destroy(erf_ctx *ctx);

@@ -25,7 +25,7 @@ ERF_VARIANT_DIFF_SPLIT = 1024
 ERF_VARIANT_FORCE_COLUMN, ERF_VARIANT_SPLIT_SLOW_RHS, ERF_VARIANT_FORCE_TILE = 4096, 8192, 16384
 
 EXPORTS = ["erf_create", "erf_set_state", "erf_rk3_step", "erf_get_state", "erf_destroy",
-           "erf_strerror", "erf_set_scalar", "erf_get_scalar", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_set_option", "erf_launch_count",
+           "erf_strerror", "erf_set_scalar", "erf_get_scalar", "erf_anelastic_step", "erf_get_pprime", "erf_project", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_set_option", "erf_launch_count",
            "erf_device_bytes", "erf_set_timing", "erf_get_timing", "erf_reset_timing", "erf_timing_name",
            "erf_measure_fp64_peak"]
 ERF_TIMING_CLASSES = 8
@@ -87,6 +87,9 @@ def load(path: str | None = None):
     L.erf_acoustic.argtypes = [C.c_void_p, C.c_double, C.c_int] + [_dp] * 10 + [C.c_void_p]
     L.erf_set_scalar.argtypes = [C.c_void_p, _dp, C.c_void_p]
     L.erf_get_scalar.argtypes = [C.c_void_p, _dp, C.c_void_p]
+    L.erf_anelastic_step.argtypes = [C.c_void_p, C.c_double, C.c_void_p]
+    L.erf_project.argtypes = [C.c_void_p, C.c_double, C.c_void_p]
+    L.erf_get_pprime.argtypes = [C.c_void_p, _dp, C.c_void_p]
     L.erf_set_path.argtypes = [C.c_void_p, C.c_int]
     L.erf_set_option.argtypes = [C.c_void_p, C.c_int, C.c_longlong]
     L.erf_launch_count.argtypes = [C.c_void_p]
@@ -154,6 +157,18 @@ def erf_set_scalar(h, rhophi, stream=None):
 
 def erf_get_scalar(h, rhophi, stream=None):
     _ck(load().erf_get_scalar(h, _ptr(rhophi), _stream(stream)), "erf_get_scalar")
+
+
+def erf_anelastic_step(h, dt, stream=None):
+    _ck(load().erf_anelastic_step(h, float(dt), _stream(stream)), "erf_anelastic_step")
+
+
+def erf_project(h, dt, stream=None):
+    _ck(load().erf_project(h, float(dt), _stream(stream)), "erf_project")
+
+
+def erf_get_pprime(h, pprime, stream=None):
+    _ck(load().erf_get_pprime(h, _ptr(pprime), _stream(stream)), "erf_get_pprime")
 
 
 def erf_destroy(h):
@@ -290,6 +305,17 @@ class Dycore:
 
     def set_scalar(self, rhophi, stream=None):
         erf_set_scalar(self._h, rhophi, stream)
+
+    def anelastic_step(self, dt, stream=None):
+        erf_anelastic_step(self._h, dt, stream)
+
+    def project(self, dt, stream=None):
+        erf_project(self._h, dt, stream)
+
+    def pprime(self, stream=None):
+        out = self.empty_state()[0]
+        erf_get_pprime(self._h, out, stream)
+        return out
 
     def get_scalar(self, stream=None):
         out = self.empty_state()[0]

@@ -37,7 +37,7 @@ extern "C" const char *erf_strerror(int code) {
   switch (code) {
     case ERF_OK: return "ok";
     case ERF_EINVAL: return "invalid argument";
-    case ERF_EUNSUPPORTED: return "unsupported configuration";
+    case ERF_EUNSUPPORTED: return "unsupported configuration (the anelastic mode needs a flat, laterally periodic grid)";
     case ERF_ENOMEM: return "out of memory";
     case ERF_ECUDA: return "CUDA error";
     default: return "unknown error";
@@ -115,6 +115,8 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   c->graph_warm = false;
   c->sc_Q = c->sc_Qt = c->sc_Qnew = c->sc_phi = c->sc_R = nullptr;
   c->sc_sum[0] = c->sc_sum[1] = c->sc_sum[2] = nullptr;
+  c->an_pp = c->an_tw = c->an_lev = nullptr;
+  c->an_w[0] = c->an_w[1] = c->an_w[2] = c->an_w[3] = nullptr;
   c->base1d_r0 = c->base1d_T0 = nullptr;
   c->zxf = c->zyf = c->zw = c->hx = c->hy = c->hc = c->zc = c->hw = c->hu = c->hv = nullptr;
   c->sxw = c->syw = c->sxu = c->syv = c->rho0 = c->Th0 = c->p0 = c->pi0 = c->Om_slow = nullptr;
@@ -284,6 +286,28 @@ extern "C" int erf_get_scalar(erf_ctx *c, double *rhophi, void *stream) {
   if (!c || !rhophi || !c->sc_Q) return ERF_EINVAL;
   if (c->status != ERF_OK) return c->status;
   cudaMemcpyAsync(rhophi, c->sc_Q, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice,
+                  (cudaStream_t)stream);
+  return check(c);
+}
+
+extern "C" int erf_anelastic_step(erf_ctx *c, double dt, void *stream) {
+  if (!c || !(dt > 0.0)) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  int rc = anelastic_step(c, dt, (cudaStream_t)stream);
+  return rc != ERF_OK ? rc : check(c);
+}
+
+extern "C" int erf_project(erf_ctx *c, double dt, void *stream) {
+  if (!c || !(dt > 0.0)) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  int rc = anelastic_project(c, c->S, dt, (cudaStream_t)stream);
+  return rc != ERF_OK ? rc : check(c);
+}
+
+extern "C" int erf_get_pprime(erf_ctx *c, double *pprime, void *stream) {
+  if (!c || !pprime || !c->an_pp) return ERF_EINVAL;
+  if (c->status != ERF_OK) return c->status;
+  cudaMemcpyAsync(pprime, c->an_pp, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice,
                   (cudaStream_t)stream);
   return check(c);
 }

@@ -53,6 +53,9 @@ struct erf_ctx {
   // erf_set_scalar
   double *sc_Q, *sc_Qt, *sc_Qnew, *sc_sum[3], *sc_phi, *sc_R;
 
+  // anelastic mode (k_anelastic.cu): lagged p', the transform work arrays, twiddle and level tables; null until first use
+  double *an_pp, *an_w[4], *an_tw, *an_lev;
+
   // ERF_OPT_GRAPH: one instantiated CUDA graph per buffer configuration of the fused step
   struct StepGraph {
     std::vector<const void *> before, after;  // buffer roles when the step starts / ends
@@ -144,7 +147,8 @@ int ensure_general(erf_ctx *c, cudaStream_t st);
 int build_general(erf_ctx *c, const gen::NodeH &Z, const double *rho0_in, const double *Th0_in, int base1d, cudaStream_t st);
 bool ensure_prim(erf_ctx *c, bool all);  // u, v, w, p' (all: also theta, pi) work arrays
 void impose_lids(erf_ctx *c, const F5 &S, cudaStream_t st);  // kinematic W on k = 0 and k = nz [R:G15]
-void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st);  // fills c->R, theta_t, pi_t
+// fills c->R, theta_t, pi_t; pan != null: the anelastic pressure-gradient / buoyancy pair with that p' (Sec. 2.2)
+void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st, const double *pan = nullptr);
 void general_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t st);  // c->P in/out
 void general_stage_init(erf_ctx *c, cudaStream_t st);    // P = S - St
 void general_stage_finish(erf_ctx *c, cudaStream_t st);  // St += P, lids
@@ -153,6 +157,10 @@ void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st);
 // k_terrain_slow.cu: the advective tendencies of all five fields in one kernel (Eq. 17-21 stencils only)
 bool terrain_advection_available(const erf_ctx *c);
 void launch_terrain_advection(erf_ctx *c, const F5 &S, cudaStream_t st);
+
+// k_anelastic.cu: RK2 + projection (Sec. 3.2 Eq. 14-16); flat, laterally periodic grids
+int anelastic_step(erf_ctx *c, double dt, cudaStream_t st);
+int anelastic_project(erf_ctx *c, const F5 &S, double dt, cudaStream_t st);
 
 // k_scalar.cu: Eq. 4 after the substeps of a stage, with the time-averaged momenta (L138)
 bool ensure_scalar(erf_ctx *c);

@@ -553,6 +553,19 @@ ERF_HD void pgbuoy_cell(const View &c, const double *const *S, const Prim &q, do
   }
 }
 
+// anelastic pair (Sec. 2.2): -grad of the projection's lagged p' and B = rho0 (theta - theta0)/theta0 g at w-faces
+ERF_HD void anel_pgbuoy_cell(const View &c, const Prim &q, const double *pan, double *const *R, int i, int j, int k) {
+  size_t a = IX(c, i, j, k);
+  R[UU][a] -= grad_x(c, pan, i, j, k);
+  R[VV][a] -= grad_y(c, pan, i, j, k);
+  if (k >= 1) {
+    size_t b = IX(c, i, j, k - 1);
+    double th0a = c.Th0[a] / c.rho0[a], th0b = c.Th0[b] / c.rho0[b];
+    double Ba = c.rho0[a] * (q.theta[a] - th0a) / th0a, Bb = c.rho0[b] * (q.theta[b] - th0b) / th0b;
+    R[WW][a] += -(pan[a] - pan[b]) / c.hw[a] + c.g * 0.5 * (Bb + Ba);
+  }
+}
+
 // ---------------------------------------------------------------- Rayleigh damping layer (L219, L622) [R:G28]
 // tau(z) = ray_coef sin^2((pi/2)(z - z_b)/ray_depth) above z_b = z_top - ray_depth (L622: sine-squared ramp from 0 at
 // the bottom of the layer to the stated inverse time scale at the top)

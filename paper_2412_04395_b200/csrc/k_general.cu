@@ -95,7 +95,7 @@ void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st) {
   launch_columns(c, st, [=] __device__(int i, int j) { gen::lids(v, U, V, W, i, j); });
 }
 
-void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st) {
+void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st, const double *pan) {
   View v = c->v;
   const int nz = c->nz;
   gen::Prim q = c->prim;
@@ -124,7 +124,10 @@ void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st) {
     launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::diff_pass7(v, d, i, j, k); });
     launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass8(v, d, R.f, i, j, k); });
   }
-  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::pgbuoy_cell(v, Sv.f, q, R.f, i, j, k); });
+  if (pan)  // anelastic mode: p' of the projection, buoyancy from theta (Sec. 2.2)
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::anel_pgbuoy_cell(v, q, pan, R.f, i, j, k); });
+  else
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::pgbuoy_cell(v, Sv.f, q, R.f, i, j, k); });
   if (v.ray_fields)  // Rayleigh damping layer (L219, L622)
     launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::rayleigh_cell(v, Sv.f, R.f, i, j, k); });
   // stage constants for the substeps: theta^t, pi^t

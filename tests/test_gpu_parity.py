@@ -554,3 +554,71 @@ def test_rayleigh_layer_matches_oracle(torch, erfo, B, cfg, kw, mask, path):
     got = _run_gpu(torch, B, case, 2, path)
     assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
     assert max(field_errors(_run_gpu(torch, B, base, 2, path), ref)) > 1e-8
+
+
+# ---------------------------------------------------------------- anelastic mode (Sec. 2.2 Eq. 8, Sec. 3.2 Eq. 14-16)
+def _numpy_divergence(case, st):
+    dz = np.diff(case["z_levels"])[:, None, None]
+    U, V, W = st[1], st[2], st[3]
+    return ((np.roll(U, -1, axis=2) - U) / case["dx"] + (np.roll(V, -1, axis=1) - V) / case["dy"] + (W[1:] - W[:-1]) / dz)
+
+
+@pytest.mark.parametrize("cfg,kw,stretch", [(1, dict(nx=40, ny=23, nz=19), 1.0), (3, dict(nx=46, ny=21, nz=34), 1.06),
+                                            (2, dict(nx=32, ny=16, nz=21), 1.0), (5, dict(nx=70, ny=11, nz=40), 1.03)])
+def test_anelastic_mode_matches_oracle(torch, erfo, B, cfg, kw, stretch):
+    """The projection alone (Eq. 16) on momenta that are far from divergence-free, then three RK2 steps (Eq. 14-15) of a
+    warm bubble in the configuration's wind, against the oracle: state, lagged p', and div(rho0 u) = 0 on the device
+    result.  Sizes include odd and non-power-of-two transform lengths; two cases have stretched levels."""
+    case = wl.make_case(cfg, **kw)
+    nz, ny, nx = case["nz"], case["ny"], case["nx"]
+    if stretch != 1.0:
+        dz = np.diff(case["z_levels"])[0] * stretch ** np.arange(nz)
+        case["z_levels"] = np.concatenate([[0.0], np.cumsum(dz)])
+    rng = np.random.default_rng(500 + cfg)
+    rho0 = np.broadcast_to(case["rho0"][:, None, None], (nz, ny, nx)).copy()
+    st = [rho0, case["state"][1] + 0.5 * rng.standard_normal((nz, ny, nx)),
+          case["state"][2] + 0.5 * rng.standard_normal((nz, ny, nx)), 0.3 * rng.standard_normal((nz + 1, ny, nx)),
+          case["state"][4].copy()]
+    st[3][0] = st[3][-1] = 0.0
+    x = (np.arange(nx) + 0.5) / nx
+    zc = (np.arange(nz) + 0.5) / nz
+    bubble = 1.5 * np.exp(-((x[None, None, :] - 0.4) / 0.15) ** 2 - ((zc[:, None, None] - 0.35) / 0.15) ** 2)
+    st[4] = st[4] + rho0 * bubble
+    dt = 4.0 * case["dt"]
+    # ---- the projection alone
+    o = erfo.Oracle(case)
+    o.set_state(*st)
+    o.project(dt)
+    ref, pref = o.get_state(), o.pprime()
+    d = B.Dycore(case)
+    d.set_state(*_dev(torch, st))
+    d.project(dt)
+    got, pgot = _host(d.get_state()), d.pprime().cpu().numpy()
+    assert max(field_errors(got, ref)) <= TOL_1STEP, field_errors(got, ref)
+    assert np.abs(pgot - pref).max() <= 1e-10 * np.abs(pref).max()
+    div0 = np.abs(_numpy_divergence(case, st)).max()
+    assert np.abs(_numpy_divergence(case, got)).max() <= 1e-11 * div0
+    # ---- three RK2 steps from the projected state (both sides continue with their own p')
+    for _ in range(3):
+        o.anelastic_step(dt)
+        d.anelastic_step(dt)
+    ref, pref = o.get_state(), o.pprime()
+    got, pgot = _host(d.get_state()), d.pprime().cpu().numpy()
+    o.close()
+    d.close()
+    assert max(field_errors(got, ref)) <= 3 * TOL_1STEP, field_errors(got, ref)
+    assert np.abs(pgot - pref).max() <= 1e-9 * np.abs(pref).max()
+    assert np.abs(_numpy_divergence(case, got)).max() <= 1e-11 * div0
+    assert np.array_equal(got[0], rho0)
+    assert np.abs(got[4] - st[4]).max() > 1e-6 * np.abs(st[4]).max()      # the bubble moved
+
+
+def test_anelastic_mode_rejects_terrain_and_open_grids(torch, B):
+    for case in (wl.make_case(4, nx=16, ny=16, nz=96), dict(wl.make_case(1, nx=16, ny=16, nz=8), periodic_x=0)):
+        d = B.Dycore(case)
+        d.set_state(*_dev(torch, case["state"]))
+        with pytest.raises(B.ErfError) as e:
+            d.anelastic_step(0.5)
+        assert e.value.code == B.ERF_EUNSUPPORTED
+        d.rk3_step(case["dt"], case["ns"])  # the context is still usable
+        d.close()
