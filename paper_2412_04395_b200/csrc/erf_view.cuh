@@ -63,4 +63,12 @@ ERF_HD size_t IX(const View &c, int i, int j, int k) {
   return ((size_t)k * c.ny + lati(j, c.ny, c.pery)) * c.nx + lati(i, c.nx, c.perx);
 }
 
+// The same view for threads whose stencils cannot leave the domain (CTAs at least a stencil width away from the lateral
+// boundary): no wrap, no clamp.  The per-cell bodies of general_cells.cuh are templates over the view type, so an
+// interior CTA runs index arithmetic that the compiler folds into constant offsets.
+struct ViewNW : View {
+  ERF_HD explicit ViewNW(const View &v) : View(v) {}
+};
+ERF_HD size_t IX(const ViewNW &c, int i, int j, int k) { return ((size_t)k * c.ny + j) * c.nx + i; }
+
 }  // namespace erfb

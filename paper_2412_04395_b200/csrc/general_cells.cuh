@@ -27,7 +27,8 @@ struct NodeH {
   }
 };
 
-ERF_HD void geo_faces(const View &c, const NodeH &Z, double *zxf, double *zyf, double *zw, int i,
+template <class VT>
+ERF_HD void geo_faces(const VT &c, const NodeH &Z, double *zxf, double *zyf, double *zw, int i,
                       int j, int k) {  // k = 0..nz
   size_t a = IX(c, i, j, k);
   zxf[a] = 0.5 * (Z(i, j, k) + Z(i, j + 1, k));
@@ -35,7 +36,8 @@ ERF_HD void geo_faces(const View &c, const NodeH &Z, double *zxf, double *zyf, d
   zw[a] = 0.25 * (Z(i, j, k) + Z(i + 1, j, k) + Z(i, j + 1, k) + Z(i + 1, j + 1, k));
 }
 
-ERF_HD void geo_cells(const View &c, const double *zxf, const double *zyf, const double *zw,
+template <class VT>
+ERF_HD void geo_cells(const VT &c, const double *zxf, const double *zyf, const double *zw,
                       double *hx, double *hy, double *hc, double *zc, int i, int j, int k) {  // k<nz
   size_t a = IX(c, i, j, k), t = IX(c, i, j, k + 1);
   hx[a] = zxf[t] - zxf[a];
@@ -44,7 +46,8 @@ ERF_HD void geo_cells(const View &c, const double *zxf, const double *zyf, const
   zc[a] = 0.5 * (zw[a] + zw[t]);
 }
 
-ERF_HD void geo_derived(const View &c, const double *zxf, const double *zyf, const double *hc,
+template <class VT>
+ERF_HD void geo_derived(const VT &c, const double *zxf, const double *zyf, const double *hc,
                         const double *zc, double *hw, double *hu, double *hv, double *sxu,
                         double *syv, double *sxw, double *syw, int i, int j, int k) {  // k = 0..nz
   size_t a = IX(c, i, j, k);
@@ -61,7 +64,8 @@ ERF_HD void geo_derived(const View &c, const double *zxf, const double *zyf, con
 }
 
 // base state p0, pi0 from Theta0 through Eq. 7 (L80) [R:S1]
-ERF_HD void base_state(const View &c, const double *rho0_in, const double *Th0_in, int base1d,
+template <class VT>
+ERF_HD void base_state(const VT &c, const double *rho0_in, const double *Th0_in, int base1d,
                        double *rho0, double *Th0, double *p0, double *pi0, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   size_t s = base1d ? (size_t)k : a;
@@ -74,7 +78,8 @@ ERF_HD void base_state(const View &c, const double *rho0_in, const double *Th0_i
 
 // ---------------------------------------------------------------- lids and Omega [R:G14,G15]
 // kinematic W on the lids: Omega = 0 there
-ERF_HD void lids(const View &c, const double *U, const double *V, double *W, int i, int j) {
+template <class VT>
+ERF_HD void lids(const VT &c, const double *U, const double *V, double *W, int i, int j) {
   int nz = c.nz;
   W[IX(c, i, j, 0)] = c.sxw[IX(c, i, j, 0)] * 0.5 * (U[IX(c, i, j, 0)] + U[IX(c, i + 1, j, 0)]) +
                       c.syw[IX(c, i, j, 0)] * 0.5 * (V[IX(c, i, j, 0)] + V[IX(c, i, j + 1, 0)]);
@@ -84,7 +89,8 @@ ERF_HD void lids(const View &c, const double *U, const double *V, double *W, int
 }
 
 // contravariant vertical mass flux (L196): Omega = W - sxw avg4(U) - syw avg4(V); 0 on lids
-ERF_HD double omega_at(const View &c, const double *U, const double *V, const double *W, int i,
+template <class VT>
+ERF_HD double omega_at(const VT &c, const double *U, const double *V, const double *W, int i,
                        int j, int k) {
   if (k < 1 || k > c.nz - 1) return 0.0;
   double ubar = 0.25 * (U[IX(c, i, j, k - 1)] + U[IX(c, i + 1, j, k - 1)] + U[IX(c, i, j, k)] +
@@ -100,7 +106,8 @@ struct Prim {
   double *theta, *pp, *pi, *u, *v, *w;
 };
 
-ERF_HD void primitives(const View &c, const double *const *S, const Prim &q, int i, int j,
+template <class VT>
+ERF_HD void primitives(const VT &c, const double *const *S, const Prim &q, int i, int j,
                        int k) {  // k = 0..nz
   size_t a = IX(c, i, j, k);
   int nz = c.nz;
@@ -190,20 +197,23 @@ ERF_HD int vertical_order(int requested, int r) {  // [R:G13]
 
 ERF_HD double sgn_of(double m) { return m < 0.0 ? -1.0 : 1.0; }  // [R:G19]
 
-ERF_HD double interp_x(const View &c, const double *f, int m, int j, int k, int order, double M) {
+template <class VT>
+ERF_HD double interp_x(const VT &c, const double *f, int m, int j, int k, int order, double M) {
   double q[6] = {0, 0, 0, 0, 0, 0};
   int half = (order % 10 + 1) / 2;
   for (int n = 3 - half; n < 3 + half; n++) q[n] = f[IX(c, m - 3 + n, j, k)];
   return interp6(order, sgn_of(M), q);
 }
-ERF_HD double interp_y(const View &c, const double *f, int i, int m, int k, int order, double M) {
+template <class VT>
+ERF_HD double interp_y(const VT &c, const double *f, int i, int m, int k, int order, double M) {
   double q[6] = {0, 0, 0, 0, 0, 0};
   int half = (order % 10 + 1) / 2;
   for (int n = 3 - half; n < 3 + half; n++) q[n] = f[IX(c, i, m - 3 + n, k)];
   return interp6(order, sgn_of(M), q);
 }
 // between levels m-1 and m; valid levels lo..hi
-ERF_HD double interp_z(const View &c, const double *f, int i, int j, int m, int lo, int hi,
+template <class VT>
+ERF_HD double interp_z(const VT &c, const double *f, int i, int j, int m, int lo, int hi,
                        int order_req, double M) {
   int below = m - lo, above = hi - m + 1;
   int r = below < above ? below : above;
@@ -216,17 +226,20 @@ ERF_HD double interp_z(const View &c, const double *f, int i, int j, int m, int 
 
 // ---------------------------------------------------------------- advection (S2)
 // mass fluxes: Fx = hx U, Fy = hy V, Omega (precomputed field Om)
-ERF_HD double FX(const View &c, const double *U, int i, int j, int k) {
+template <class VT>
+ERF_HD double FX(const VT &c, const double *U, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   return c.hx[a] * U[a];
 }
-ERF_HD double FY(const View &c, const double *V, int i, int j, int k) {
+template <class VT>
+ERF_HD double FY(const VT &c, const double *V, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   return c.hy[a] * V[a];
 }
 
 // R_rho, R_Theta, R_U, R_V at cell (i,j,k), k < nz   (Eq. 1-3 first terms; L196)
-ERF_HD void advect_cell(const View &c, const double *const *S, const double *Om, const Prim &q,
+template <class VT>
+ERF_HD void advect_cell(const VT &c, const double *const *S, const double *Om, const Prim &q,
                         double *const *R, int i, int j, int k) {
   const int nz = c.nz, oh = c.oh, ov = c.ov;
   const double *U = S[UU], *V = S[VV];
@@ -279,7 +292,8 @@ ERF_HD void advect_cell(const View &c, const double *const *S, const double *Om,
 }
 
 // R_W at face (i,j,k), k = 0..nz (zero on the lids)
-ERF_HD void advect_wface(const View &c, const double *const *S, const double *Om, const Prim &q,
+template <class VT>
+ERF_HD void advect_wface(const VT &c, const double *const *S, const double *Om, const Prim &q,
                          double *const *R, int i, int j, int k) {
   const int nz = c.nz, oh = c.oh, ov = c.ov;
   const double *U = S[UU], *V = S[VV];
@@ -315,7 +329,8 @@ struct Diff {
 };
 
 // mean of the valid (k' in 1..nz-1) quotients at levels k, k+1 and two columns [R:G14]
-ERF_HD double avg_q_valid(const View &c, const double *qv, int i0, int j0, int i1, int j1, int k) {
+template <class VT>
+ERF_HD double avg_q_valid(const VT &c, const double *qv, int i0, int j0, int i1, int j1, int k) {
   double s = 0.0;
   int n = 0;
   for (int kk = k; kk <= k + 1; kk++)
@@ -327,7 +342,8 @@ ERF_HD double avg_q_valid(const View &c, const double *qv, int i0, int j0, int i
 }
 
 // pass D1: qu, qv (k = 1..nz-1; 0 elsewhere), S33 (k < nz)
-ERF_HD void diff_pass1(const View &c, const Prim &q, const Diff &d, int i, int j, int k) {
+template <class VT>
+ERF_HD void diff_pass1(const VT &c, const Prim &q, const Diff &d, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   if (k >= 1 && k <= c.nz - 1) {
     size_t b = IX(c, i, j, k - 1);
@@ -343,7 +359,8 @@ ERF_HD void diff_pass1(const View &c, const Prim &q, const Diff &d, int i, int j
 }
 
 // pass D2: S11, S22, S12 (k < nz); S13, S23 (k = 1..nz-1, 0 on the lids)
-ERF_HD void diff_pass2(const View &c, const Prim &q, const Diff &d, int i, int j, int k) {
+template <class VT>
+ERF_HD void diff_pass2(const VT &c, const Prim &q, const Diff &d, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   const double dx = c.dx, dy = c.dy;
   if (k < c.nz) {
@@ -394,7 +411,8 @@ ERF_HD void diff_pass2(const View &c, const Prim &q, const Diff &d, int i, int j
 }
 
 // pass D3: mu, K at centres (k < nz).  Smagorinsky-Lilly [R:G9]; mu_m = rho nu [R:G10]
-ERF_HD void diff_pass3(const View &c, const double *rhof, const Diff &d, int i, int j, int k) {
+template <class VT>
+ERF_HD void diff_pass3(const VT &c, const double *rhof, const Diff &d, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   double rho = rhof[a];
   double mu = rho * c.nu, K = rho * c.alpha;
@@ -416,7 +434,8 @@ ERF_HD void diff_pass3(const View &c, const double *rhof, const Diff &d, int i, 
 }
 
 // pass D4: stresses tau = -2 mu sigma (Eq. 9) and the xy-edge height (k < nz; t13,t23 = 0 at k = 0, nz)
-ERF_HD void diff_pass4(const View &c, const Diff &d, int i, int j, int k) {
+template <class VT>
+ERF_HD void diff_pass4(const VT &c, const Diff &d, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   if (k >= c.nz) {
     d.t13[a] = 0.0;
@@ -443,7 +462,8 @@ ERF_HD void diff_pass4(const View &c, const Diff &d, int i, int j, int k) {
 }
 
 // pass D5: vertical two-point quotients of the stresses and of theta (chain rule) [R:G14]
-ERF_HD void diff_pass5(const View &c, const Prim &q, const Diff &d, int i, int j, int k) {  // k<nz
+template <class VT>
+ERF_HD void diff_pass5(const VT &c, const Prim &q, const Diff &d, int i, int j, int k) {  // k<nz
   size_t a = IX(c, i, j, k);
   if (k >= 1) {
     size_t b = IX(c, i, j, k - 1);
@@ -465,7 +485,8 @@ ERF_HD void diff_pass5(const View &c, const Prim &q, const Diff &d, int i, int j
 }
 
 // pass D6: momentum R -= div tau; horizontal scalar fluxes Fx, Fy (k < nz)
-ERF_HD void diff_pass6(const View &c, const Prim &q, const Diff &d, double *const *R, int i, int j,
+template <class VT>
+ERF_HD void diff_pass6(const VT &c, const Prim &q, const Diff &d, double *const *R, int i, int j,
                        int k) {
   size_t a = IX(c, i, j, k);
   const double dx = c.dx, dy = c.dy;
@@ -504,7 +525,8 @@ ERF_HD void diff_pass6(const View &c, const Prim &q, const Diff &d, double *cons
 }
 
 // pass D7: contravariant vertical scalar flux at w-faces, k = 0..nz (0 on lids)
-ERF_HD void diff_pass7(const View &c, const Diff &d, int i, int j, int k) {
+template <class VT>
+ERF_HD void diff_pass7(const VT &c, const Diff &d, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   if (k < 1 || k > c.nz - 1) {
     d.Fz[a] = 0.0;
@@ -518,30 +540,35 @@ ERF_HD void diff_pass7(const View &c, const Diff &d, int i, int j, int k) {
 }
 
 // pass D8: R_Theta -= div F (k < nz)
-ERF_HD void diff_pass8(const View &c, const Diff &d, double *const *R, int i, int j, int k) {
+template <class VT>
+ERF_HD void diff_pass8(const VT &c, const Diff &d, double *const *R, int i, int j, int k) {
   size_t a = IX(c, i, j, k), ip = IX(c, i + 1, j, k), jp = IX(c, i, j + 1, k), kp = IX(c, i, j, k + 1);
   R[TH][a] -= ((c.hx[ip] * d.Fx[ip] - c.hx[a] * d.Fx[a]) / c.dx + (c.hy[jp] * d.Fy[jp] - c.hy[a] * d.Fy[a]) / c.dy +
                (d.Fz[kp] - d.Fz[a])) / c.hc[a];
 }
 
 // ---------------------------------------------------------------- pressure gradient, buoyancy (S4)
-ERF_HD double dz_centre(const View &c, const double *f, int i, int j, int k) {
+template <class VT>
+ERF_HD double dz_centre(const VT &c, const double *f, int i, int j, int k) {
   int kb = k > 0 ? k - 1 : 0;
   int kt = k < c.nz - 1 ? k + 1 : c.nz - 1;
   return (f[IX(c, i, j, kt)] - f[IX(c, i, j, kb)]) / (c.zc[IX(c, i, j, kt)] - c.zc[IX(c, i, j, kb)]);
 }
-ERF_HD double grad_x(const View &c, const double *f, int i, int j, int k) {
+template <class VT>
+ERF_HD double grad_x(const VT &c, const double *f, int i, int j, int k) {
   double along = (f[IX(c, i, j, k)] - f[IX(c, i - 1, j, k)]) / c.dx;
   if (c.nz == 1 || c.flat) return along;
   return along - c.sxu[IX(c, i, j, k)] * 0.5 * (dz_centre(c, f, i - 1, j, k) + dz_centre(c, f, i, j, k));
 }
-ERF_HD double grad_y(const View &c, const double *f, int i, int j, int k) {
+template <class VT>
+ERF_HD double grad_y(const VT &c, const double *f, int i, int j, int k) {
   double along = (f[IX(c, i, j, k)] - f[IX(c, i, j - 1, k)]) / c.dy;
   if (c.nz == 1 || c.flat) return along;
   return along - c.syv[IX(c, i, j, k)] * 0.5 * (dz_centre(c, f, i, j - 1, k) + dz_centre(c, f, i, j, k));
 }
 
-ERF_HD void pgbuoy_cell(const View &c, const double *const *S, const Prim &q, double *const *R, int i,
+template <class VT>
+ERF_HD void pgbuoy_cell(const VT &c, const double *const *S, const Prim &q, double *const *R, int i,
                         int j, int k) {  // k < nz
   size_t a = IX(c, i, j, k);
   R[UU][a] -= grad_x(c, q.pp, i, j, k);
@@ -554,7 +581,8 @@ ERF_HD void pgbuoy_cell(const View &c, const double *const *S, const Prim &q, do
 }
 
 // anelastic pair (Sec. 2.2): -grad of the projection's lagged p' and B = rho0 (theta - theta0)/theta0 g at w-faces
-ERF_HD void anel_pgbuoy_cell(const View &c, const Prim &q, const double *pan, double *const *R, int i, int j, int k) {
+template <class VT>
+ERF_HD void anel_pgbuoy_cell(const VT &c, const Prim &q, const double *pan, double *const *R, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   R[UU][a] -= grad_x(c, pan, i, j, k);
   R[VV][a] -= grad_y(c, pan, i, j, k);
@@ -577,7 +605,8 @@ ERF_HD double rayleigh_tau(double depth, double coef, double z, double ztop) {
 }
 
 // relaxation of the masked primitives towards their references (u_ref, v_ref, 0, theta0), k < nz
-ERF_HD void rayleigh_cell(const View &c, const double *const *S, double *const *R, int i, int j, int k) {
+template <class VT>
+ERF_HD void rayleigh_cell(const VT &c, const double *const *S, double *const *R, int i, int j, int k) {
   const int nz = c.nz, f = c.ray_fields;
   const size_t a = IX(c, i, j, k), t = IX(c, i, j, nz);
   if (f & 1) {
@@ -608,7 +637,8 @@ struct Acou {
 };
 
 // step 1: Theta''_d = Theta'' + beta_d (Theta'' - Theta''_prev); prev <- Theta''
-ERF_HD void ac_damp(const View &c, const Acou &A, int i, int j, int k) {
+template <class VT>
+ERF_HD void ac_damp(const VT &c, const Acou &A, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   double T = A.P[TH][a];
   A.Thd[a] = T + c.beta_d * (T - A.Th_prev[a]);
@@ -616,7 +646,8 @@ ERF_HD void ac_damp(const View &c, const Acou &A, int i, int j, int k) {
 }
 
 // step 2: explicit horizontal momenta (L585 rows 1-2)
-ERF_HD void ac_horiz(const View &c, const Acou &A, double dtau, int i, int j, int k) {
+template <class VT>
+ERF_HD void ac_horiz(const VT &c, const Acou &A, double dtau, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   double gR = c.gam * c.Rd;
   double piu = 0.5 * (A.pi_t[IX(c, i - 1, j, k)] + A.pi_t[a]);
@@ -632,7 +663,8 @@ ERF_HD void ac_horiz(const View &c, const Acou &A, double dtau, int i, int j, in
 }
 
 // step 3: omega = sxw avg4(U''new) + syw avg4(V''new), k = 1..nz-1 [R:G16]
-ERF_HD void ac_slope(const View &c, const Acou &A, int i, int j, int k) {
+template <class VT>
+ERF_HD void ac_slope(const VT &c, const Acou &A, int i, int j, int k) {
   size_t a = IX(c, i, j, k);
   if (k < 1 || k > c.nz - 1) {
     A.om[a] = 0.0;
@@ -647,7 +679,8 @@ ERF_HD void ac_slope(const View &c, const Acou &A, int i, int j, int k) {
 // steps 4-6: one column.  Forward sweep builds the explicit parts, the rows of the
 // tridiagonal system for Omega''new (L144; S5) and eliminates; backward sweep
 // substitutes and updates W'', Theta'', rho'' (L585 rows 3-5, L591).
-ERF_HD void ac_column(const View &c, const Acou &A, double dtau, int i, int j) {
+template <class VT>
+ERF_HD void ac_column(const VT &c, const Acou &A, double dtau, int i, int j) {
   const int nz = c.nz;
   const double b1 = 0.5 * (1.0 - c.beta_s), b2 = 0.5 * (1.0 + c.beta_s);  // L589
   const double g = c.g, gR = c.gam * c.Rd;

@@ -95,16 +95,74 @@ void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st) {
   launch_columns(c, st, [=] __device__(int i, int j) { gen::lids(v, U, V, W, i, j); });
 }
 
+// ---- per-cell passes as functors over the view type: CTAs whose 32 x 8 tile lies at least MARGIN columns inside the
+// domain run the body on a ViewNW (no wrap / clamp in the index helper), the others on the View
+namespace {
+constexpr int MARGIN = 3;
+
+template <class F>
+__global__ void __launch_bounds__(256) k_cells_v(View v, int nlev, F f) {
+  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k = blockIdx.z;
+  if (i >= v.nx || j >= v.ny || k >= nlev) return;
+  const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8;
+  const bool inner = x0 >= MARGIN && x0 + 32 + MARGIN <= v.nx && y0 >= MARGIN && y0 + 8 + MARGIN <= v.ny;
+  if (inner) {
+    const ViewNW vn(v);
+    f(vn, i, j, k);
+  } else {
+    f(v, i, j, k);
+  }
+}
+
+template <class F>
+void launch_cells_v(erf_ctx *c, cudaStream_t st, int nlev, const F &f) {
+  if (nlev <= 0) return;
+  dim3 block(32, 8), grid((c->nx + 31) / 32, (c->ny + 7) / 8, nlev);
+  k_cells_v<<<grid, block, 0, st>>>(c->v, nlev, f);
+  c->launches++;
+}
+
+struct FPrim {
+  F5 S; gen::Prim q;
+  template <class VT> __device__ void operator()(const VT &v, int i, int j, int k) const { gen::primitives(v, S.f, q, i, j, k); }
+};
+struct FOmega {
+  F5 S; double *Om;
+  template <class VT> __device__ void operator()(const VT &v, int i, int j, int k) const {
+    Om[IX(v, i, j, k)] = gen::omega_at(v, S.f[UU], S.f[VV], S.f[WW], i, j, k);
+  }
+};
+template <int PASS>
+struct FDiff {
+  gen::Prim q; gen::Diff d; F5 R; const double *rho;
+  template <class VT> __device__ void operator()(const VT &v, int i, int j, int k) const {
+    if (PASS == 1) gen::diff_pass1(v, q, d, i, j, k);
+    if (PASS == 2) gen::diff_pass2(v, q, d, i, j, k);
+    if (PASS == 3) gen::diff_pass3(v, rho, d, i, j, k);
+    if (PASS == 4) gen::diff_pass4(v, d, i, j, k);
+    if (PASS == 5) gen::diff_pass5(v, q, d, i, j, k);
+    if (PASS == 6) gen::diff_pass6(v, q, d, R.f, i, j, k);
+    if (PASS == 7) gen::diff_pass7(v, d, i, j, k);
+    if (PASS == 8) gen::diff_pass8(v, d, R.f, i, j, k);
+  }
+};
+struct FPgBuoy {
+  F5 S, R; gen::Prim q; const double *pan;
+  template <class VT> __device__ void operator()(const VT &v, int i, int j, int k) const {
+    if (pan) gen::anel_pgbuoy_cell(v, q, pan, R.f, i, j, k);  // anelastic mode: p' of the projection, buoyancy from theta
+    else gen::pgbuoy_cell(v, S.f, q, R.f, i, j, k);
+  }
+};
+}  // namespace
+
 void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st, const double *pan) {
   View v = c->v;
   const int nz = c->nz;
   gen::Prim q = c->prim;
   F5 Sv = S, R = c->R;
   double *Om = c->Om_slow;
-  launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::primitives(v, Sv.f, q, i, j, k); });
-  launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) {
-    Om[IX(v, i, j, k)] = gen::omega_at(v, Sv.f[UU], Sv.f[VV], Sv.f[WW], i, j, k);
-  });
+  launch_cells_v(c, st, nz + 1, FPrim{Sv, q});
+  launch_cells_v(c, st, nz + 1, FOmega{Sv, Om});
   if (c->path == ERF_PATH_AUTO && terrain_advection_available(c)) {
     launch_terrain_advection(c, S, st);  // all five advective tendencies in one kernel (k_terrain_slow.cu)
   } else {
@@ -115,19 +173,16 @@ void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st, const double *pa
     if (!ensure_diff(c)) return;
     gen::Diff d = c->diff;
     const double *rho = S.f[RHO];
-    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::diff_pass1(v, q, d, i, j, k); });
-    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::diff_pass2(v, q, d, i, j, k); });
-    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass3(v, rho, d, i, j, k); });
-    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::diff_pass4(v, d, i, j, k); });
-    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass5(v, q, d, i, j, k); });
-    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass6(v, q, d, R.f, i, j, k); });
-    launch_cells(c, st, nz + 1, [=] __device__(int i, int j, int k) { gen::diff_pass7(v, d, i, j, k); });
-    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::diff_pass8(v, d, R.f, i, j, k); });
+    launch_cells_v(c, st, nz + 1, FDiff<1>{q, d, R, rho});
+    launch_cells_v(c, st, nz + 1, FDiff<2>{q, d, R, rho});
+    launch_cells_v(c, st, nz, FDiff<3>{q, d, R, rho});
+    launch_cells_v(c, st, nz + 1, FDiff<4>{q, d, R, rho});
+    launch_cells_v(c, st, nz, FDiff<5>{q, d, R, rho});
+    launch_cells_v(c, st, nz, FDiff<6>{q, d, R, rho});
+    launch_cells_v(c, st, nz + 1, FDiff<7>{q, d, R, rho});
+    launch_cells_v(c, st, nz, FDiff<8>{q, d, R, rho});
   }
-  if (pan)  // anelastic mode: p' of the projection, buoyancy from theta (Sec. 2.2)
-    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::anel_pgbuoy_cell(v, q, pan, R.f, i, j, k); });
-  else
-    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::pgbuoy_cell(v, Sv.f, q, R.f, i, j, k); });
+  launch_cells_v(c, st, nz, FPgBuoy{Sv, R, q, pan});
   if (v.ray_fields)  // Rayleigh damping layer (L219, L622)
     launch_cells(c, st, nz, [=] __device__(int i, int j, int k) { gen::rayleigh_cell(v, Sv.f, R.f, i, j, k); });
   // stage constants for the substeps: theta^t, pi^t
