@@ -102,9 +102,10 @@ constexpr int MARGIN = 3;
 
 template <class F>
 __global__ void __launch_bounds__(256) k_cells_v(View v, int nlev, F f) {
-  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k = blockIdx.z;
+  // levels fastest in the launch order (vertical neighbours of the resident CTAs stay in L2)
+  const int i = blockIdx.y * 32 + threadIdx.x, j = blockIdx.z * 8 + threadIdx.y, k = blockIdx.x;
   if (i >= v.nx || j >= v.ny || k >= nlev) return;
-  const int x0 = blockIdx.x * 32, y0 = blockIdx.y * 8;
+  const int x0 = blockIdx.y * 32, y0 = blockIdx.z * 8;
   const bool inner = x0 >= MARGIN && x0 + 32 + MARGIN <= v.nx && y0 >= MARGIN && y0 + 8 + MARGIN <= v.ny;
   if (inner) {
     const ViewNW vn(v);
@@ -117,7 +118,7 @@ __global__ void __launch_bounds__(256) k_cells_v(View v, int nlev, F f) {
 template <class F>
 void launch_cells_v(erf_ctx *c, cudaStream_t st, int nlev, const F &f) {
   if (nlev <= 0) return;
-  dim3 block(32, 8), grid((c->nx + 31) / 32, (c->ny + 7) / 8, nlev);
+  dim3 block(32, 8), grid(nlev, (c->nx + 31) / 32, (c->ny + 7) / 8);
   k_cells_v<<<grid, block, 0, st>>>(c->v, nlev, f);
   c->launches++;
 }

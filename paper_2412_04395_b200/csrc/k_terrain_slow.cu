@@ -6,7 +6,7 @@
 //   theta, u, v, w (L196) and the stencils of Eq. 17-21 (L198-L211) in the branch-free form
 //   flux = M q_even - |M| q_odd [R:G1], vertical order reduced next to the lids [R:G13].
 //
-// One thread per cell, one level per blockIdx.z (so the vertical order is uniform over a CTA).  The seven column
+// One thread per cell, one level per CTA (so the vertical order is uniform over a CTA).  The seven column
 // offsets in x and in y are wrapped (periodic) or clamped (open boundary) once per thread; every stencil value is then one load at
 // level base + row offset + column offset, served by L1/L2 (neighbouring threads share all but one point).  This
 // replaces the two terrain-general advection passes (general_cells.cuh advect_cell / advect_wface: a run-time
@@ -33,7 +33,8 @@ __device__ __forceinline__ double hdiv(const double *q, double Mm, double Mp) {
 
 template <int OH>
 __global__ void __launch_bounds__(256) k_adv_terrain(const Args p) {
-  const int i = blockIdx.x * 32 + threadIdx.x, j = blockIdx.y * 8 + threadIdx.y, k = blockIdx.z;
+  // levels fastest in the launch order: the CTAs resident at one time share their +-3 level windows through L2
+  const int i = blockIdx.y * 32 + threadIdx.x, j = blockIdx.z * 8 + threadIdx.y, k = blockIdx.x;
   const int nx = p.nx, ny = p.ny, nz = p.nz;
   if (i >= nx || j >= ny) return;
   const size_t plane = (size_t)nx * ny, kb = (size_t)k * plane;
@@ -150,7 +151,7 @@ void launch_terrain_advection(erf_ctx *c, const F5 &S, cudaStream_t st) {
   p.Rrho = c->R.f[RHO]; p.RU = c->R.f[UU]; p.RV = c->R.f[VV]; p.RW = c->R.f[WW]; p.RTh = c->R.f[TH];
   p.nx = c->nx; p.ny = c->ny; p.nz = c->nz; p.ov = v.ov; p.perx = v.perx; p.pery = v.pery;
   p.rdx = 1.0 / v.dx; p.rdy = 1.0 / v.dy;
-  dim3 block(32, 8), grid((c->nx + 31) / 32, (c->ny + 7) / 8, c->nz);
+  dim3 block(32, 8), grid(c->nz, (c->nx + 31) / 32, (c->ny + 7) / 8);
   switch (v.oh) {
     case 2: tslow::k_adv_terrain<2><<<grid, block, 0, st>>>(p); break;
     case 3: tslow::k_adv_terrain<3><<<grid, block, 0, st>>>(p); break;
