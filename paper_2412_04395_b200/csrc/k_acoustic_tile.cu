@@ -294,10 +294,12 @@ static void launch_mode(const AcArgs &p, dim3 grid, int chunk, size_t smem, cuda
 
 // Which substep kernel.  Splitting the levels of a column over the warps of a CTA exposes nz / 16 times more parallelism
 // per column than one thread per column, which wins while the grid has too few columns to fill the machine (measured on
-// B200, substeps per RK3 step: 32x32x32 0.15 against 0.39 ms, 128x128x64 0.74 against 1.44 ms); on large grids the
-// CTAs of this kernel touch one 256-byte row on every level of every field at once and the thread-per-column kernel,
-// which sweeps the domain plane by plane, is faster (256x256x128: 6.6 against 3.9 ms; 1024x1024x128: 104.6 against
-// 59.1 ms per step) although it moves 27 % more bytes.  Developer knobs: ERF_VARIANT_FORCE_TILE / _FORCE_COLUMN.
+// B200, substeps per RK3 step: 32x32x32 0.15 against 0.39 ms, 128x128x64 0.74 against 1.44 ms).  On large grids the
+// thread-per-column kernel is faster (256x256x128: 3.9 against 6.6 ms; 1024x1024x128: 59.1 against 104.6 ms per step)
+// although it moves 27 % more bytes: both kernels are bound by load latency at 16 warps per SM, and the tile kernel adds
+// two barriers, a single-warp phase and a second pass over its levels (profiles/r2_substep_experiments.md; addressing the
+// fields as [j][k][i] instead of [k][j][i] does not change its time, so the layout is not the reason).
+// Developer knobs: ERF_VARIANT_FORCE_TILE / _FORCE_COLUMN.
 bool acoustic_tile_selected(const erf_ctx *c) {
   if (!c->fz || !c->fz->ok || (c->fz->variant & ERF_VARIANT_FORCE_COLUMN)) return false;
   if (actile::smem_bytes(c->nz) > 226 * 1024) return false;  // 3 nz rows of 32 columns: nz <= 290
