@@ -12,10 +12,9 @@
 //     [lx(m) + ly(n)] P_k + [ (P_{k+1} - P_k)/hw_{k+1} - (P_k - P_{k-1})/hw_k ] / dz_k = Dhat_k / dt,
 //     lx(m) = -(4/dx^2) sin^2(pi m / nx), ly(n) = -(4/dy^2) sin^2(pi n / ny);  mode (0, 0): psi_hat(k = 0) = 0.
 //
-// Kernels.  The transforms are direct sums over a twiddle table (one output per thread; x: the row staged in shared
-// memory, y: coalesced column reads).  That is O(n) work per output: fine for the grids this mode is tested on, and the
-// one place of this file where a radix-2 kernel would replace the sum for power-of-two sizes.  The column solve is one
-// thread per mode (m, n), Thomas in place, real and imaginary part together.
+// Kernels.  Power-of-two lengths: radix-2 transforms in shared memory (x: one row per CTA; y: eight neighbouring columns
+// of a level per CTA).  Other lengths: direct sums over the twiddle table, one output per thread (O(n) work per output).
+// The column solve is one thread per mode (m, n), Thomas in place, real and imaginary part together.
 #include "erf_ctx.cuh"
 
 namespace erfb {
@@ -96,6 +95,80 @@ __global__ void k_dft_y(int nx, int ny, const double *__restrict__ ar, const dou
   }
   br[kb + (size_t)n * nx + m] = sr;
   bi[kb + (size_t)n * nx + m] = si;
+}
+
+// ---- power-of-two lengths: radix-2 transforms in shared memory (decimation in time: bit-reversed load, log2 n butterfly
+// stages with the twiddles of the table).  NB sequences of length n per CTA, sequence b at re/im[b * n ...].
+template <int SIGN>
+__device__ __forceinline__ void fft_stages(double *re, double *im, int n, int logn, int nb, const double *tc,
+                                           const double *ts, int tid, int nthr) {
+  const int half_n = n >> 1;
+  for (int s = 1; s <= logn; s++) {
+    const int len = 1 << s, half = len >> 1, tstep = n >> s;
+    __syncthreads();
+    for (int t = tid; t < nb * half_n; t += nthr) {
+      const int b = t / half_n, q = t - b * half_n;
+      const int grp = q / half, pos = q - grp * half;
+      const int i0 = b * n + grp * len + pos, i1 = i0 + half;
+      const double wr = tc[pos * tstep], wi = SIGN * ts[pos * tstep];
+      const double xr = re[i1] * wr - im[i1] * wi, xi = re[i1] * wi + im[i1] * wr;
+      const double ar = re[i0], ai = im[i0];
+      re[i0] = ar + xr; im[i0] = ai + xi;
+      re[i1] = ar - xr; im[i1] = ai - xi;
+    }
+  }
+  __syncthreads();
+}
+
+// x: one (j, k) row per CTA; ai may be null (real input), bi may be null (real output)
+template <int SIGN>
+__global__ void k_fft_x(int nx, int logn, const double *__restrict__ ar, const double *__restrict__ ai, double *br,
+                        double *bi, const double *__restrict__ tw, double scale) {
+  extern __shared__ double sm[];
+  double *re = sm, *im = sm + nx, *tc = sm + 2 * nx, *ts = sm + 3 * nx;
+  const size_t row = (size_t)blockIdx.x * nx;
+  for (int t = threadIdx.x; t < nx; t += blockDim.x) {
+    const int r = (int)(__brev((unsigned)t) >> (32 - logn));
+    re[r] = ar[row + t];
+    im[r] = ai ? ai[row + t] : 0.0;
+    tc[t] = tw[t];
+    ts[t] = tw[nx + t];
+  }
+  fft_stages<SIGN>(re, im, nx, logn, 1, tc, ts, threadIdx.x, blockDim.x);
+  for (int t = threadIdx.x; t < nx; t += blockDim.x) {
+    br[row + t] = re[t] * scale;
+    if (bi) bi[row + t] = im[t] * scale;
+  }
+}
+
+// y: NB = 8 neighbouring columns m of one level per CTA
+template <int SIGN>
+__global__ void k_fft_y(int nx, int ny, int logn, const double *__restrict__ ar, const double *__restrict__ ai,
+                        double *br, double *bi, const double *__restrict__ tw) {
+  constexpr int NB = 8;
+  extern __shared__ double sm[];
+  double *re = sm, *im = sm + NB * ny, *tc = sm + 2 * NB * ny, *ts = tc + ny;
+  const int m0 = blockIdx.x * NB, k = blockIdx.y, tid = threadIdx.x, nthr = blockDim.x;
+  const size_t kb = (size_t)k * nx * ny;
+  for (int t = tid; t < ny; t += nthr) { tc[t] = tw[t]; ts[t] = tw[ny + t]; }
+  for (int t = tid; t < NB * ny; t += nthr) {
+    const int b = t % NB, j = t / NB;  // b fastest: 64-byte segments of a row
+    if (m0 + b < nx) {
+      const int r = (int)(__brev((unsigned)j) >> (32 - logn));
+      re[b * ny + r] = ar[kb + (size_t)j * nx + m0 + b];
+      im[b * ny + r] = ai[kb + (size_t)j * nx + m0 + b];
+    } else {
+      re[b * ny + j] = 0.0; im[b * ny + j] = 0.0;
+    }
+  }
+  fft_stages<SIGN>(re, im, ny, logn, NB, tc, ts, tid, nthr);
+  for (int t = tid; t < NB * ny; t += nthr) {
+    const int b = t % NB, n = t / NB;
+    if (m0 + b < nx) {
+      br[kb + (size_t)n * nx + m0 + b] = re[b * ny + n];
+      bi[kb + (size_t)n * nx + m0 + b] = im[b * ny + n];
+    }
+  }
 }
 
 // one tridiagonal system per mode: lev = [dz(0..nz-1) | hw(0..nz), hw(0) unused]; (br, bi) in/out; cp = scratch c'
@@ -199,8 +272,16 @@ int anelastic_project(erf_ctx *c, const F5 &S, double dt, cudaStream_t st) {
   const int tx = nx < 256 ? ((nx + 31) / 32) * 32 : 256;
   const size_t smx = 4 * (size_t)nx * sizeof(double), smy = 2 * (size_t)ny * sizeof(double);
   if (smx > 200 * 1024 || smy > 200 * 1024) return ERF_EUNSUPPORTED;
+  auto log2i = [](int n) { int l = 0; while ((1 << l) < n) l++; return ((1 << l) == n && n >= 2) ? l : -1; };
+  const int lx = log2i(nx), ly = log2i(ny);  // -1: not a power of two, the direct sums run
+  const size_t smfy = (size_t)(2 * 8 + 2) * ny * sizeof(double);
+  const int tfx = nx / 2 < 256 ? (nx / 2 < 32 ? 32 : nx / 2) : 256;
   static bool attr = false;
   if (!attr) {
+    cudaFuncSetAttribute(anel::k_fft_x<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(anel::k_fft_x<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(anel::k_fft_y<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    cudaFuncSetAttribute(anel::k_fft_y<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(anel::k_dft_x<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(anel::k_dft_x<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(anel::k_dft_y<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -208,11 +289,17 @@ int anelastic_project(erf_ctx *c, const F5 &S, double dt, cudaStream_t st) {
     attr = true;
   }
   anel::k_div<<<grid, block, 0, st>>>(c->v, S.f[UU], S.f[VV], S.f[WW], c->an_lev, Br);
-  anel::k_dft_x<-1><<<ny * nz, tx, smx, st>>>(nx, Br, nullptr, Ar, Ai, twx, 1.0);
-  anel::k_dft_y<-1><<<grid, block, smy, st>>>(nx, ny, Ar, Ai, Br, Bi, twy);
+  const bool fy = ly > 0 && smfy <= 200 * 1024;
+  dim3 gfy((nx + 7) / 8, nz);
+  if (lx > 0) anel::k_fft_x<-1><<<ny * nz, tfx, smx, st>>>(nx, lx, Br, nullptr, Ar, Ai, twx, 1.0);
+  else anel::k_dft_x<-1><<<ny * nz, tx, smx, st>>>(nx, Br, nullptr, Ar, Ai, twx, 1.0);
+  if (fy) anel::k_fft_y<-1><<<gfy, 256, smfy, st>>>(nx, ny, ly, Ar, Ai, Br, Bi, twy);
+  else anel::k_dft_y<-1><<<grid, block, smy, st>>>(nx, ny, Ar, Ai, Br, Bi, twy);
   anel::k_modes<<<gmodes, block, 0, st>>>(nx, ny, nz, c->v.dx, c->v.dy, 1.0 / dt, c->an_lev, Br, Bi, Ar);
-  anel::k_dft_y<1><<<grid, block, smy, st>>>(nx, ny, Br, Bi, Ar, Ai, twy);
-  anel::k_dft_x<1><<<ny * nz, tx, smx, st>>>(nx, Ar, Ai, Br, nullptr, twx, 1.0 / ((double)nx * ny));
+  if (fy) anel::k_fft_y<1><<<gfy, 256, smfy, st>>>(nx, ny, ly, Br, Bi, Ar, Ai, twy);
+  else anel::k_dft_y<1><<<grid, block, smy, st>>>(nx, ny, Br, Bi, Ar, Ai, twy);
+  if (lx > 0) anel::k_fft_x<1><<<ny * nz, tfx, smx, st>>>(nx, lx, Ar, Ai, Br, nullptr, twx, 1.0 / ((double)nx * ny));
+  else anel::k_dft_x<1><<<ny * nz, tx, smx, st>>>(nx, Ar, Ai, Br, nullptr, twx, 1.0 / ((double)nx * ny));
   anel::k_correct<<<grid, block, 0, st>>>(c->v, Br, c->an_lev, dt, S.f[UU], S.f[VV], S.f[WW], c->an_pp);
   c->launches += 7;
   return c->status;

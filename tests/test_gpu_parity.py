@@ -564,11 +564,14 @@ def _numpy_divergence(case, st):
 
 
 @pytest.mark.parametrize("cfg,kw,stretch", [(1, dict(nx=40, ny=23, nz=19), 1.0), (3, dict(nx=46, ny=21, nz=34), 1.06),
-                                            (2, dict(nx=32, ny=16, nz=21), 1.0), (5, dict(nx=70, ny=11, nz=40), 1.03)])
+                                            (2, dict(nx=32, ny=16, nz=21), 1.0), (5, dict(nx=70, ny=11, nz=40), 1.03),
+                                            (3, dict(nx=64, ny=128, nz=12), 1.0), (1, dict(nx=2, ny=4, nz=6), 1.0),
+                                            (2, dict(nx=40, ny=32, nz=9), 1.0)])
 def test_anelastic_mode_matches_oracle(torch, erfo, B, cfg, kw, stretch):
     """The projection alone (Eq. 16) on momenta that are far from divergence-free, then three RK2 steps (Eq. 14-15) of a
     warm bubble in the configuration's wind, against the oracle: state, lagged p', and div(rho0 u) = 0 on the device
-    result.  Sizes include odd and non-power-of-two transform lengths; two cases have stretched levels."""
+    result.  Sizes include odd and non-power-of-two transform lengths (direct sums) and powers of two (radix-2
+    kernels), also mixed; two cases have stretched levels."""
     case = wl.make_case(cfg, **kw)
     nz, ny, nx = case["nz"], case["ny"], case["nx"]
     if stretch != 1.0:
