@@ -219,7 +219,7 @@ def time_config(binding, wl, torch, config, steps, warmup, repeats, graph, devic
            "value": cells / (ms * 1e-3), "launches_per_step": launches, "launch": "cuda_graph" if graph else "stream",
            "algorithmic_bytes_per_cell": ad["total"] * 8,
            "whole_step_frac": ad["total"] * 8 * cells / (ms * 1e-3) / 1e9 / peak,
-           "path": "fused flat kernels" if case.get("z_nodes") is None else "terrain: general slow RHS + fused terrain substeps",
+           "path": "fused flat kernels" if case.get("z_nodes") is None else "terrain: fused advection + general diffusion passes + fused terrain substeps",
            "repeats": repeats, "steps": steps, "device_bytes": dyc.device_bytes}
     dyc.close()
     del dev
