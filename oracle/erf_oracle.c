@@ -42,6 +42,8 @@ enum { RHO = 0, UU = 1, VV = 2, WW = 3, TH = 4 };
 struct erfo_ctx {
   int nx, ny, nz;
   int perx, pery; /* lateral boundary per direction: 1 periodic, 0 open */
+  int inx, iny;   /* inflow: the first column (row) of cells is held at the values given to erfo_set_state [R:G30] */
+  double *inflow[5];
   int flat;       /* z_nodes == NULL: level heights depend on k only */
   double dx, dy;
   erfo_params p;
@@ -312,6 +314,22 @@ static void build_geometry(erfo_ctx *c, const double *zn) {
       }
   fill_lateral(c, c->sxw);
   fill_lateral(c, c->syw);
+}
+
+/* Inflow boundary ("inflow", Table C1 "Inflow, Outflow"; no discrete form in the paper) [R:G30]: the
+ * first column of cells at the low-x side -- rho, rho*theta, rho*v, rho*w of cell i = 0 and rho*u on its low face,
+ * which is the boundary face -- is held at the values the state was given (erfo_set_state): a Dirichlet column.  Beyond
+ * it the open closure applies (ghost = nearest interior value = the inflow value); the far side is open (outflow).
+ * Imposed on every stage result; likewise in y. */
+static void impose_inflow(const erfo_ctx *c, double *const S[5]) {
+  if (c->inx)
+    for (int m = 0; m < 5; m++)
+      for (int k = 0; k <= c->nz; k++)
+        for (int j = 0; j < c->ny; j++) S[m][IX(c, 0, j, k)] = c->inflow[m][IX(c, 0, j, k)];
+  if (c->iny)
+    for (int m = 0; m < 5; m++)
+      for (int k = 0; k <= c->nz; k++)
+        for (int i = 0; i < c->nx; i++) S[m][IX(c, i, 0, k)] = c->inflow[m][IX(c, i, 0, k)];
 }
 
 /* ------------------------------------------------------------------ */
@@ -1318,6 +1336,7 @@ int erfo_rk3_step(erfo_ctx *c, double dt, int n_acoustic) {
       for (int m = 0; m < 5; m++) /* L593 */
         for (size_t a = 0; a < c->n; a++) St[m][a] = St[m][a] + P[m][a];
     }
+    impose_inflow(c, St);
     for (int m = 0; m < 5; m++) fill_lateral(c, St[m]);
     impose_lids(c, St[UU], St[VV], St[WW]);
   }
@@ -1563,7 +1582,8 @@ int erfo_create(const erfo_grid *g, const erfo_metrics *m, const erfo_params *p,
     return -1;
   erfo_ctx *c = (erfo_ctx *)calloc(1, sizeof(erfo_ctx));
   c->nx = g->nx; c->ny = g->ny; c->nz = g->nz; c->dx = g->dx; c->dy = g->dy;
-  c->perx = g->periodic_x != 0; c->pery = g->periodic_y != 0;
+  c->perx = g->periodic_x == 1; c->pery = g->periodic_y == 1;
+  c->inx = g->periodic_x == 2; c->iny = g->periodic_y == 2;
   c->flat = m->z_nodes == NULL;
   c->p = *p;
   c->cv = p->cp - p->Rd;
@@ -1613,6 +1633,7 @@ void erfo_destroy(erfo_ctx *c) {
   for (size_t a = 0; a < sizeof(all) / sizeof(all[0]); a++) free(all[a]);
   free(c->Q);
   free(c->pan);
+  for (int m = 0; m < 5; m++) free(c->inflow[m]);
   free(c);
 }
 
@@ -1625,6 +1646,11 @@ int erfo_set_state(erfo_ctx *c, const double *rho, const double *rhou, const dou
   put_dense(c, c->S[WW], rhow, c->nz + 1);
   put_dense(c, c->S[TH], rhotheta, c->nz);
   impose_lids(c, c->S[UU], c->S[VV], c->S[WW]);
+  if (c->inx || c->iny)
+    for (int m = 0; m < 5; m++) {
+      if (!c->inflow[m]) c->inflow[m] = fnew(c);
+      memcpy(c->inflow[m], c->S[m], c->n * sizeof(double));
+    }
   return 0;
 }
 

@@ -30,7 +30,8 @@ typedef struct erfo_ctx erfo_ctx;
 typedef struct {
   int nx, ny, nz;
   double dx, dy;
-  int periodic_x, periodic_y; /* per direction: 1 periodic (L229); 0 open = zero normal gradient [R:G27] */
+  int periodic_x, periodic_y; /* per direction: 1 periodic (L229); 0 open = zero normal gradient [R:G27];
+                                 2 inflow at the low side (a Dirichlet column of cells [R:G30]), open at the high side */
 } erfo_grid;
 
 typedef struct {

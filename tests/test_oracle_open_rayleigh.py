@@ -174,3 +174,47 @@ def test_rayleigh_layer_damps_w_at_the_stated_rate():
     assert W[1][k, 0, 0] / W[0][k, 0, 0] == pytest.approx(1 + z + z * z / 2 + z ** 3 / 6, rel=1e-7)
     assert abs(W[1][k, 0, 0] / W[0][k, 0, 0] - 1.0) > 1e-4
     assert np.array_equal(W[1][10], W[0][10])       # below the layer nothing is damped
+
+
+# ------------------------------------------------------------------ inflow (reading G30: a Dirichlet column of cells)
+def test_inflow_column_is_held_and_feeds_the_domain():
+    """periodic_x = 2: the first column of cells keeps the values it was given, exactly, whatever happens inside; what
+    it holds is carried into the domain by the wind.  A column 1 K warmer than the rest at a 20 m/s inflow: after 60 s
+    the warm air has reached x = u t = 1200 m (cell 12) -- warm well behind the front, untouched well ahead of it.  With
+    the open closure (periodic_x = 0) nothing holds the boundary column: its value floats with the flow."""
+    nx, dx, u0 = 48, 100.0, 20.0
+    case = uniform_case(nx, 3, 6, dx, dx, 100.0, adv_order_h=3, adv_order_v=3)
+    dth = np.zeros((6, 3, nx))
+    dth[:, :, 0] = 1.0
+    st = _state(case, u=u0, dtheta=dth)
+    r0, t0 = base_state_fields(case)
+    res = {}
+    for code in (2, 0):
+        case["periodic_x"] = code
+        o = erfo.Oracle(case)
+        o.set_state(*st)
+        for _ in range(60):
+            o.step(1.0, 6)
+        got = o.get_state()
+        res[code] = got[4] / got[0] - t0 / r0
+        if code == 2:
+            for f in range(5):
+                assert np.array_equal(got[f][..., 0], st[f][..., 0]), f     # the Dirichlet column, bitwise
+    th = res[2][2, 1]
+    assert th[1:7].min() > 0.9 and th[1:7].max() < 1.1        # behind the front: the inflow value
+    assert abs(th[12] - 0.5) < 0.35                           # the front is where u t says
+    assert np.abs(th[24:]).max() < 1e-3                       # ahead of it: nothing yet
+    assert abs(res[0][2, 1][0] - 1.0) > 0.05                  # open closure: the boundary value is not held, it floats
+
+
+@pytest.mark.parametrize("code", [(2, 1), (1, 2), (2, 2), (2, 0)])
+def test_uniform_flow_is_steady_with_inflow(code):
+    case = uniform_case(12, 9, 6, 100.0, 80.0, 50.0, adv_order_h=5, adv_order_v=5, diffusion=1, nu=2.0, alpha_theta=2.0)
+    case["periodic_x"], case["periodic_y"] = code
+    st = _state(case, u=7.0, v=3.0)
+    o = erfo.Oracle(case)
+    o.set_state(*st)
+    for _ in range(3):
+        o.step(0.5, 4)
+    for a, b in zip(o.get_state(), st):
+        assert np.abs(a - b).max() <= 1e-11 * max(np.abs(b).max(), 1.0)
