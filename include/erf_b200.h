@@ -49,7 +49,10 @@ typedef struct {
   double dx, dy;              /* m, uniform (L178) */
   int periodic_x, periodic_y; /* per direction: 1 periodic; 0 open (L229 "periodic, inflow, outflow, or open"):
                                  every ghost value is the nearest interior value (zero normal gradient,
-                                 DESIGN.md reading G27); open grids run the terrain-general kernels      */
+                                 DESIGN.md reading G27); 2 inflow at the low side, open (outflow) at the high
+                                 side: the first column of cells -- rho*u on the boundary face included -- is
+                                 held at the values given to erf_set_state (reading G30); non-periodic grids
+                                 run the terrain-general kernels                                           */
 } erf_grid;
 
 typedef struct {

@@ -61,6 +61,7 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   *out = nullptr;
   if (g->nx < 1 || g->ny < 1 || g->nz < 1 || !(g->dx > 0) || !(g->dy > 0)) return ERF_EINVAL;
   if (!m->rho0 || !m->rhotheta0 || (!m->z_nodes && !m->z_levels)) return ERF_EINVAL;
+  if (g->periodic_x < 0 || g->periodic_x > 2 || g->periodic_y < 0 || g->periodic_y > 2) return ERF_EINVAL;
   if (p->adv_order_h < 2 || p->adv_order_h > 6 || p->adv_order_v < 2 || p->adv_order_v > 6) return ERF_EINVAL;
   if (p->diffusion < 0 || p->diffusion > 2 || (p->substep_mode != 0 && p->substep_mode != 1)) return ERF_EINVAL;
   if (!(p->cp > p->Rd) || !(p->Rd > 0) || !(p->p00 > 0)) return ERF_EINVAL;
@@ -99,7 +100,9 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   v.osh = p->scalar_adv ? p->scalar_adv : p->adv_order_h;
   v.osv = p->scalar_adv ? p->scalar_adv : p->adv_order_v;
   v.flat = m->z_nodes ? 0 : 1;
-  v.perx = g->periodic_x != 0; v.pery = g->periodic_y != 0;
+  v.perx = g->periodic_x == 1; v.pery = g->periodic_y == 1;
+  c->inx = g->periodic_x == 2; c->iny = g->periodic_y == 2;
+  c->in_x = c->in_y = nullptr;
   v.ray_fields = p->ray_depth > 0.0 && p->ray_coef > 0.0 ? p->ray_fields : 0;
   v.ray_depth = p->ray_depth; v.ray_coef = p->ray_coef; v.ray_uref = p->ray_uref; v.ray_vref = p->ray_vref;
   v.dx = g->dx; v.dy = g->dy;
@@ -180,6 +183,7 @@ extern "C" int erf_set_state(erf_ctx *c, const double *rho, const double *rhou, 
   cudaMemcpyAsync(c->S.f[WW], rhow, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
   cudaMemcpyAsync(c->S.f[TH], rhotheta, nc, cudaMemcpyDeviceToDevice, st);
   impose_lids(c, c->S, st);
+  inflow_store(c, st);
   return check(c);
 }
 
@@ -403,6 +407,7 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
         for (int f = 0; f < 5; f++)
           if (f == WW || k < v.nz) St.f[f][a] = S.f[f][a] + dts * R.f[f][a];
       });
+      inflow_impose(c, c->St, st);
       impose_lids(c, c->St, st);
     } else {
       {

@@ -53,6 +53,10 @@ struct erf_ctx {
   // erf_set_scalar
   double *sc_Q, *sc_Qt, *sc_Qnew, *sc_sum[3], *sc_phi, *sc_R;
 
+  // inflow boundaries [R:G30]: the Dirichlet column i = 0 ([5][nz+1][ny]) / row j = 0 ([5][nz+1][nx]) given to erf_set_state
+  int inx, iny;
+  double *in_x, *in_y;
+
   // anelastic mode (k_anelastic.cu): lagged p', the transform work arrays, twiddle and level tables; null until first use
   double *an_pp, *an_w[4], *an_tw, *an_lev;
 
@@ -153,6 +157,8 @@ void general_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t
 void general_stage_init(erf_ctx *c, cudaStream_t st);    // P = S - St
 void general_stage_finish(erf_ctx *c, cudaStream_t st);  // St += P, lids
 void general_lids(erf_ctx *c, const F5 &S, cudaStream_t st);
+void inflow_store(erf_ctx *c, cudaStream_t st);                  // remember column / row 0 of c->S
+void inflow_impose(erf_ctx *c, const F5 &S, cudaStream_t st);    // write it back into S (every stage result)
 
 // k_terrain_slow.cu: the advective tendencies of all five fields in one kernel (Eq. 17-21 stencils only)
 bool terrain_advection_available(const erf_ctx *c);

@@ -156,6 +156,45 @@ struct FPgBuoy {
 };
 }  // namespace
 
+// ---- inflow boundary [R:G30]: the first column (row) of cells is a Dirichlet column held at the values of erf_set_state
+__global__ void k_inflow(F5 S, double *in_x, double *in_y, int nx, int ny, int nz, bool store) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y, f = blockIdx.z;
+  const size_t plane = (size_t)nx * ny;
+  if (in_x && t < ny) {
+    const size_t a = (size_t)k * plane + (size_t)t * nx, b = ((size_t)f * (nz + 1) + k) * ny + t;
+    if (store) in_x[b] = S.f[f][a]; else S.f[f][a] = in_x[b];
+  }
+  if (in_y && t < nx) {
+    const size_t a = (size_t)k * plane + t, b = ((size_t)f * (nz + 1) + k) * nx + t;
+    if (store) in_y[b] = S.f[f][a]; else S.f[f][a] = in_y[b];
+  }
+}
+
+static void inflow_launch(erf_ctx *c, const F5 &S, bool store, cudaStream_t st) {
+  const int n = c->nx > c->ny ? c->nx : c->ny;
+  dim3 grid((n + 127) / 128, c->nz + 1, 5);
+  if (!store && c->in_x && c->in_y) {  // x first, then y (the corner holds the same stored value either way)
+    k_inflow<<<grid, 128, 0, st>>>(S, c->in_x, nullptr, c->nx, c->ny, c->nz, false);
+    k_inflow<<<grid, 128, 0, st>>>(S, nullptr, c->in_y, c->nx, c->ny, c->nz, false);
+    c->launches += 2;
+    return;
+  }
+  k_inflow<<<grid, 128, 0, st>>>(S, c->in_x, c->in_y, c->nx, c->ny, c->nz, store);
+  c->launches++;
+}
+
+void inflow_store(erf_ctx *c, cudaStream_t st) {
+  if (!c->inx && !c->iny) return;
+  if (c->inx && !c->in_x) c->in_x = c->alloc((size_t)5 * (c->nz + 1) * c->ny);
+  if (c->iny && !c->in_y) c->in_y = c->alloc((size_t)5 * (c->nz + 1) * c->nx);
+  if (c->status != ERF_OK) return;
+  inflow_launch(c, c->S, true, st);
+}
+
+void inflow_impose(erf_ctx *c, const F5 &S, cudaStream_t st) {
+  if ((c->inx && c->in_x) || (c->iny && c->in_y)) inflow_launch(c, S, false, st);
+}
+
 void general_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st, const double *pan) {
   View v = c->v;
   const int nz = c->nz;
@@ -219,6 +258,7 @@ void general_stage_finish(erf_ctx *c, cudaStream_t st) {
     }
     St.f[WW][a] += P.f[WW][a];
   });
+  inflow_impose(c, c->St, st);
   general_lids(c, c->St, st);
 }
 

@@ -501,12 +501,13 @@ def test_weno_scalars_match_oracle(torch, erfo, B, cfg, kw, code):
 
 
 # ---------------------------------------------------------------- open lateral boundaries (L229) and Rayleigh layer (L219, L622)
-@pytest.mark.parametrize("per", [(0, 1), (1, 0), (0, 0)])
+@pytest.mark.parametrize("per", [(0, 1), (1, 0), (0, 0), (2, 1), (0, 2), (2, 2)])
 @pytest.mark.parametrize("cfg,kw", [(2, dict(nx=38, ny=19, nz=21)), (5, dict(nx=70, ny=11, nz=40)),
                                     (4, dict(nx=44, ny=36, nz=96))])
 def test_open_boundaries_match_oracle(torch, erfo, B, cfg, kw, per):
-    """Open (zero normal gradient) lateral boundaries in x, in y and in both: f(S) of a developed state and two full
-    steps against the oracle, on flat crops and over the hill (the hill sits away from the boundary)."""
+    """Open (0: zero normal gradient) and inflow (2: a held column of cells, open far side) lateral boundaries in x, in y
+    and in both: f(S) of a developed state and two full steps against the oracle, on flat crops and over the hill
+    (the hill sits away from the boundary); an inflow column must come back bitwise."""
     case = wl.make_case(cfg, **kw)
     case["periodic_x"], case["periodic_y"] = per
     st = _run_oracle(erfo, case, 1)
@@ -523,6 +524,12 @@ def test_open_boundaries_match_oracle(torch, erfo, B, cfg, kw, per):
     ref = _run_oracle(erfo, case, 2)
     got = _run_gpu(torch, B, case, 2)
     assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
+    if per[0] == 2:
+        for f in (0, 1, 2, 4):
+            assert np.array_equal(got[f][..., 0], case["state"][f][..., 0]), f
+    if per[1] == 2:
+        for f in (0, 1, 2, 4):
+            assert np.array_equal(got[f][:, 0, :], case["state"][f][:, 0, :]), f
     # the open closure is not the periodic one
     per_case = dict(case, periodic_x=1, periodic_y=1)
     assert max(field_errors(_run_gpu(torch, B, per_case, 2), ref)) > 1e-9
