@@ -118,8 +118,9 @@ int erf_get_state(erf_ctx *ctx, double *rho, double *rhou, double *rhov, double 
 /* One transported scalar phi (Eq. 4), passed and returned as rho*phi, DEVICE [nz][ny][nx].  Once set,
  * every erf_rk3_step advances it in each RK stage AFTER the acoustic substeps, advected by the time average over
  * the stage of the normal momenta that advanced rho in the substeps (L138) -- so a constant phi stays constant --
- * and diffused with theta's diffusivity.  A context that carries a scalar runs the terrain-general kernels
- * (ERF_PATH_GENERAL) for the whole step.  erf_get_scalar before erf_set_scalar: ERF_EINVAL. */
+ * and diffused with theta's diffusivity.  The dycore keeps its path (on flat periodic grids the fused substep kernel
+ * accumulates the averaged momenta); the scalar's own stage runs on the terrain-general kernels, whose 3-D metric arrays
+ * erf_set_scalar allocates.  erf_get_scalar before erf_set_scalar: ERF_EINVAL. */
 int erf_set_scalar(erf_ctx *ctx, const double *rhophi, void *cuda_stream);
 int erf_get_scalar(erf_ctx *ctx, double *rhophi, void *cuda_stream);
 

@@ -15,6 +15,7 @@ struct AcArgs {
   const double *Pu, *Pv, *Pw, *Pr, *Pt, *Ptp;  // S'' in: U'', V'', W'', rho'', Theta'' and Theta''_prev
   const double *Sn[5], *St[5];                 // FIRST: S'' = Sn - St;  LAST: St is added to the result
   double *oU, *oV, *oW, *oR, *oT, *oTp;        // out: S'' (or the stage result); oTp: initial Theta'' (FIRST)
+  double *sumU, *sumV, *sumOm;                 // null, or the sums over the substeps of the momenta that advance rho'' (L138)
   double *kW, *kR, *kT, *cp_scr;               // column scratch between the sweeps (thread-per-column kernel)
   const double *RU, *RV, *RW, *Rrho, *RTh;
   const double *theta, *pi, *iT;

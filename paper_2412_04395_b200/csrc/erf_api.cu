@@ -117,7 +117,7 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   c->graph_on = false;
   c->graph_warm = false;
   c->sc_Q = c->sc_Qt = c->sc_Qnew = c->sc_phi = c->sc_R = nullptr;
-  c->sc_sum[0] = c->sc_sum[1] = c->sc_sum[2] = nullptr;
+  c->sc_sum[0] = c->sc_sum[1] = c->sc_sum[2] = c->sc_G[0] = c->sc_G[1] = nullptr;
   c->an_pp = c->an_tw = c->an_lev = nullptr;
   c->an_w[0] = c->an_w[1] = c->an_w[2] = c->an_w[3] = nullptr;
   c->base1d_r0 = c->base1d_T0 = nullptr;
@@ -274,8 +274,8 @@ extern "C" const char *erf_timing_name(int id) {
 extern "C" long long erf_launch_count(const erf_ctx *c) { return c ? c->launches : 0; }
 extern "C" long long erf_device_bytes(const erf_ctx *c) { return c ? c->bytes : 0; }
 
-// (a context with a transported scalar runs the terrain-general kernels, which accumulate the averaged momenta)
-static bool use_fused(const erf_ctx *c) { return c->path == ERF_PATH_AUTO && fused_available(c) && !c->sc_Q; }
+// (with a transported scalar the fused substep kernel accumulates the averaged momenta: k_acoustic_flat<.., ACC>)
+static bool use_fused(const erf_ctx *c) { return c->path == ERF_PATH_AUTO && fused_available(c); }
 
 extern "C" int erf_set_scalar(erf_ctx *c, const double *rhophi, void *stream) {
   if (!c || !rhophi) return ERF_EINVAL;
@@ -380,7 +380,7 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
   if (c->status != ERF_OK) return c->status;
   cudaStream_t st = (cudaStream_t)stream;
   if (use_fused(c)) {
-    if (c->graph_on && !c->timing) return graph_step(c, dt, n_acoustic, st);
+    if (c->graph_on && !c->timing && !c->sc_Q) return graph_step(c, dt, n_acoustic, st);
     fused_rk3_step(c, dt, n_acoustic, st);
     return check(c);
   }

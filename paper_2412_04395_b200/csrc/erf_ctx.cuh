@@ -51,7 +51,7 @@ struct erf_ctx {
 
   // one transported scalar (k_scalar.cu): rho*phi, its stage values, the sums of the substep momenta; null until
   // erf_set_scalar
-  double *sc_Q, *sc_Qt, *sc_Qnew, *sc_sum[3], *sc_phi, *sc_R;
+  double *sc_Q, *sc_Qt, *sc_Qnew, *sc_sum[3], *sc_phi, *sc_R, *sc_G[2];
 
   // inflow boundaries [R:G30]: the Dirichlet column i = 0 ([5][nz+1][ny]) / row j = 0 ([5][nz+1][nx]) given to erf_set_state
   int inx, iny;
@@ -171,7 +171,8 @@ int anelastic_project(erf_ctx *c, const F5 &S, double dt, cudaStream_t st);
 // k_scalar.cu: Eq. 4 after the substeps of a stage, with the time-averaged momenta (L138)
 bool ensure_scalar(erf_ctx *c);
 void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, double *Qout, int nsub, double dts,
-                  cudaStream_t st);
+                  cudaStream_t st, bool folded = false);
+void scalar_prepare_fused(erf_ctx *c, const F5 &St, const double *Qt, int nsub, cudaStream_t st);
 
 // k_acoustic_terrain.cu: general_acoustic with the per-substep passes fused (terrain grids)
 bool terrain_acoustic_available(const erf_ctx *c);

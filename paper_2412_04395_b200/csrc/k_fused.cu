@@ -142,7 +142,8 @@ void fused_slow_rhs(erf_ctx *c, const F5 &S, cudaStream_t st) { launch_slow_flat
 static void acoustic_substeps(erf_ctx *c, double dtau, int n, int stage, cudaStream_t st) {
   FusedState *z = c->fz;
   if (n <= 0) return;
-  const bool tile = acoustic_tile_selected(c);
+  const bool acc = c->sc_Q != nullptr && stage >= 1;  // transported scalar: accumulate the averaged momenta (L138)
+  const bool tile = acoustic_tile_selected(c) && !acc;
   AcArgs p;
   p.nx = c->nx; p.ny = c->ny; p.nz = c->nz;
   p.dtau = dtau; p.rdx = 1.0 / c->v.dx; p.rdy = 1.0 / c->v.dy;
@@ -152,6 +153,7 @@ static void acoustic_substeps(erf_ctx *c, double dtau, int n, int stage, cudaStr
   p.theta = c->theta_t; p.pi = c->pi_t; p.iT = z->iT;
   p.rdz = z->tab.rdz; p.rhw = z->tab.rhw; p.tabB = z->tab.tabB;
   p.cp_scr = z->cp_scr;
+  p.sumU = acc ? c->sc_sum[0] : nullptr; p.sumV = acc ? c->sc_sum[1] : nullptr; p.sumOm = acc ? c->sc_sum[2] : nullptr;
 
   double *cur = c->P.f[TH], *prev = c->P.f[TH], *fr[2] = {z->Thd[0], z->Thd[1]};  // the three Theta'' buffers
   int nfree = 2;
@@ -228,13 +230,22 @@ void fused_acoustic(erf_ctx *c, const F5 &St, double dtau, int n, cudaStream_t s
 }
 
 void fused_rk3_step(erf_ctx *c, double dt, int ns, cudaStream_t st) {
+  if (c->sc_Q) cudaMemcpyAsync(c->sc_Qt, c->sc_Q, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
   for (int stage = 1; stage <= 3; stage++) {
     int nsub = stage == 1 ? 1 : (stage == 2 ? ns / 2 : ns);  // L170
     double dtau = stage == 1 ? dt / 3.0 : dt / ns;
+    const double dts = stage == 1 ? dt / 3.0 : (stage == 2 ? dt / 2.0 : dt);
     // f(S^t) every stage (L140) (also theta^t, pi^t, 1/Theta^t); S^t = S^n in stage 1
-    launch_slow_flat(c, stage == 1 ? c->S : c->St, st);
+    const F5 &Sstage = stage == 1 ? c->S : c->St;
+    launch_slow_flat(c, Sstage, st);
+    if (c->sc_Q) scalar_prepare_fused(c, Sstage, c->sc_Qt, nsub, st);  // before the last substep overwrites S^t
     acoustic_substeps(c, dtau, nsub, stage, st);
+    if (c->sc_Q) {  // Eq. 4 after the substeps of the stage (L138)
+      scalar_stage(c, c->St, c->sc_Qt, c->sc_Q, c->sc_Qnew, nsub, dts, st, true);
+      double *t = c->sc_Qt; c->sc_Qt = c->sc_Qnew; c->sc_Qnew = t;
+    }
   }
+  if (c->sc_Q) { double *t = c->sc_Q; c->sc_Q = c->sc_Qt; c->sc_Qt = t; }
   for (int f = 0; f < 5; f++) {
     double *t = c->S.f[f];
     c->S.f[f] = c->St.f[f];

@@ -36,7 +36,9 @@ struct FwdIn {
   double om_t, RW, rpp, RTh, Rrho, iT, sU, sV;
 };
 
-template <int ROWS, int MODE>
+// ACC: also accumulate the momenta of this substep's continuity equation -- U''new, V''new and beta2 Omega''new + beta1
+// Omega''old -- for the transported scalars (Eq. 4 with the stage-time-averaged momenta, L138; k_scalar.cu)
+template <int ROWS, int MODE, bool ACC>
 __global__ void __launch_bounds__(32 * ROWS, 4) k_acoustic_flat(const AcArgs p) {
   constexpr bool FIRST = (MODE & MODE_FIRST) != 0, LAST = (MODE & MODE_LAST) != 0, ZERO = (MODE & MODE_ZERO) != 0;
   constexpr int BD = 4;
@@ -150,6 +152,11 @@ __global__ void __launch_bounds__(32 * ROWS, 4) k_acoustic_flat(const AcArgs p) 
     }
     p.oU[a] = LAST ? cur.sU + Um : Um;
     p.oV[a] = LAST ? cur.sV + Vm : Vm;
+    if (ACC) {
+      p.sumU[a] += Um;
+      p.sumV[a] += Vm;
+      if (k >= 1) p.sumOm[a] += b1 * om_b;  // the old-time part of the vertical flux (L591); the new-time part below
+    }
     if (FIRST && !LAST && !ZERO) p.oTp[a] = cur.d_c;  // Theta''_prev of the next substep
     p.kT[a] = Ttil;  // parked
     p.kR[a] = rtil;  // parked
@@ -210,6 +217,7 @@ __global__ void __launch_bounds__(32 * ROWS, 4) k_acoustic_flat(const AcArgs p) 
         const double rhc = rdz[k];
         const double Tnew = bc.Ttil - cb * (thft * On_t - thfb * On_b) * rhc;
         const double rnew = bc.rtil - cb * (On_t - On_b) * rhc;
+        if (ACC && k >= 1) p.sumOm[a] += b2 * On_b;
         if (LAST) {
           p.oW[a] = k >= 1 ? bc.sW + On_b : 0.0;  // L593; flat lid: W = 0 at k = 0
           p.oT[a] = bc.sT + Tnew;
@@ -227,16 +235,22 @@ __global__ void __launch_bounds__(32 * ROWS, 4) k_acoustic_flat(const AcArgs p) 
   }
 }
 
-void launch_acoustic_flat_one(const AcArgs &p, int mode, cudaStream_t st) {
+template <bool ACC>
+static void launch_acc(const AcArgs &p, int mode, cudaStream_t st) {
   constexpr int ROWS = 4;
   dim3 block(32, ROWS), grid((p.nx + 31) / 32, (p.ny + ROWS - 1) / ROWS);
   switch (mode) {
-    case 0: k_acoustic_flat<ROWS, 0><<<grid, block, 0, st>>>(p); break;
-    case MODE_FIRST: k_acoustic_flat<ROWS, MODE_FIRST><<<grid, block, 0, st>>>(p); break;
-    case MODE_LAST: k_acoustic_flat<ROWS, MODE_LAST><<<grid, block, 0, st>>>(p); break;
-    case MODE_FIRST | MODE_LAST: k_acoustic_flat<ROWS, MODE_FIRST | MODE_LAST><<<grid, block, 0, st>>>(p); break;
-    default: k_acoustic_flat<ROWS, MODE_FIRST | MODE_LAST | MODE_ZERO><<<grid, block, 0, st>>>(p); break;
+    case 0: k_acoustic_flat<ROWS, 0, ACC><<<grid, block, 0, st>>>(p); break;
+    case MODE_FIRST: k_acoustic_flat<ROWS, MODE_FIRST, ACC><<<grid, block, 0, st>>>(p); break;
+    case MODE_LAST: k_acoustic_flat<ROWS, MODE_LAST, ACC><<<grid, block, 0, st>>>(p); break;
+    case MODE_FIRST | MODE_LAST: k_acoustic_flat<ROWS, MODE_FIRST | MODE_LAST, ACC><<<grid, block, 0, st>>>(p); break;
+    default: k_acoustic_flat<ROWS, MODE_FIRST | MODE_LAST | MODE_ZERO, ACC><<<grid, block, 0, st>>>(p); break;
   }
+}
+
+void launch_acoustic_flat_one(const AcArgs &p, int mode, cudaStream_t st) {
+  if (p.sumU) launch_acc<true>(p, mode, st);
+  else launch_acc<false>(p, mode, st);
 }
 
 }  // namespace erfb

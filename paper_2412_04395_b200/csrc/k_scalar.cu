@@ -9,9 +9,12 @@
 // (general_cells.cuh: ac_horiz, ac_column).  With them a constant phi stays constant to round-off.  phi is interpolated
 // like theta (Eq. 17-21, order reduction at the lids [R:G13]); it diffuses with theta's K, conservative form [R:G25].
 //
-// Round 2: runs on the terrain-general data path (thread per cell, mass fluxes and vertical quotients formed on
-// the fly); a context with a scalar takes the general kernels for the whole step.
-#include "erf_ctx.cuh"
+// The scalar stage itself runs on the terrain-general data path (thread per cell, mass fluxes and vertical quotients
+// formed on the fly).  The momenta come from the substep kernels of whichever path runs the step: the general passes, or
+// the fused flat-grid kernel k_acoustic_flat<.., ACC = true>.  On the fused path the last substep of a stage overwrites
+// the stage state, so there the sums are started at n times the stage momenta ("folded") and phi^t is formed before the
+// substeps (scalar_prepare_fused); the stage then needs nothing of S^t.
+#include "fused.cuh"
 
 namespace erfb {
 
@@ -22,6 +25,7 @@ struct Sc {
   const double *rho, *U, *V, *W;     // stage state S^t
   const double *Us, *Vs, *Oms;       // sums over the substeps (null without substepping)
   double rn;                         // 1 / number of substeps
+  bool folded;                       // the sums already hold n times the stage momenta (U, V, W are null)
   const double *Qt, *Qn, *K;
   double *phi, *Gx, *Gy, *R, *Qout;
   double dts;
@@ -29,14 +33,17 @@ struct Sc {
 
 __device__ __forceinline__ double mx(const Sc &s, int i, int j, int k) {  // averaged mass flux through x-face i
   const size_t a = IX(s.v, i, j, k);
+  if (s.folded) return s.v.hx[a] * (s.rn * s.Us[a]);
   return s.v.hx[a] * (s.U[a] + (s.Us ? s.rn * s.Us[a] : 0.0));
 }
 __device__ __forceinline__ double my(const Sc &s, int i, int j, int k) {
   const size_t a = IX(s.v, i, j, k);
+  if (s.folded) return s.v.hy[a] * (s.rn * s.Vs[a]);
   return s.v.hy[a] * (s.V[a] + (s.Vs ? s.rn * s.Vs[a] : 0.0));
 }
 __device__ __forceinline__ double mz(const Sc &s, int i, int j, int k) {  // averaged Omega through w-face k
   if (k < 1 || k > s.v.nz - 1) return 0.0;
+  if (s.folded) return s.rn * s.Oms[IX(s.v, i, j, k)];  // flat grid: Omega = W
   return gen::omega_at(s.v, s.U, s.V, s.W, i, j, k) + (s.Oms ? s.rn * s.Oms[IX(s.v, i, j, k)] : 0.0);
 }
 
@@ -69,21 +76,24 @@ __device__ __forceinline__ double gy_at(const Sc &s, int i, int j, int k) {
 
 // Q_stage from Q^t (stage value) and Q^n; nsub = 0: no substepping (the stage momenta advect)
 void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, double *Qout, int nsub, double dts,
-                  cudaStream_t st) {
+                  cudaStream_t st, bool folded) {
   Sc s;
   s.v = c->v;
+  s.folded = folded;
   s.rho = St.f[RHO]; s.U = St.f[UU]; s.V = St.f[VV]; s.W = St.f[WW];
   s.Us = nsub ? c->sc_sum[0] : nullptr; s.Vs = nsub ? c->sc_sum[1] : nullptr; s.Oms = nsub ? c->sc_sum[2] : nullptr;
   s.rn = nsub ? 1.0 / nsub : 0.0;
-  s.Qt = Qt; s.Qn = Qn; s.K = c->p.diffusion != 0 ? c->diff.K : nullptr;
-  s.phi = c->sc_phi; s.R = c->sc_R; s.Gx = c->diff.Fx; s.Gy = c->diff.Fy; s.Qout = Qout;
+  s.Qt = Qt; s.Qn = Qn; s.K = c->p.diffusion != 0 ? (folded ? c->fz->Kd : c->diff.K) : nullptr;
+  s.phi = c->sc_phi; s.R = c->sc_R; s.Qout = Qout;
+  s.Gx = folded ? c->sc_G[0] : c->diff.Fx; s.Gy = folded ? c->sc_G[1] : c->diff.Fy;
   s.dts = dts;
   const int nz = c->nz;
   const bool diffuse = c->p.diffusion != 0;
-  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
-    const size_t a = IX(s.v, i, j, k);
-    s.phi[a] = s.Qt[a] / s.rho[a];
-  });
+  if (!folded)
+    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
+      const size_t a = IX(s.v, i, j, k);
+      s.phi[a] = s.Qt[a] / s.rho[a];
+    });
   launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
     const View &v = s.v;
     const size_t a = IX(v, i, j, k);
@@ -121,10 +131,28 @@ void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, 
   });
 }
 
+// fused flat path, before the substeps of a stage: phi^t = Q^t / rho^t and the sums started at n times the stage momenta
+void scalar_prepare_fused(erf_ctx *c, const F5 &St, const double *Qt, int nsub, cudaStream_t st) {
+  const View v = c->v;
+  const double *rho = St.f[RHO], *U = St.f[UU], *V = St.f[VV], *W = St.f[WW];
+  double *phi = c->sc_phi, *sU = c->sc_sum[0], *sV = c->sc_sum[1], *sO = c->sc_sum[2];
+  const double n = (double)nsub;
+  launch_cells(c, st, c->nz + 1, [=] __device__(int i, int j, int k) {
+    const size_t a = IX(v, i, j, k);
+    if (k < v.nz) {
+      phi[a] = Qt[a] / rho[a];
+      sU[a] = n * U[a];
+      sV[a] = n * V[a];
+    }
+    sO[a] = n * W[a];
+  });
+}
+
 // first use: the scalar, its two stage buffers, the three momentum sums and two work arrays
 bool ensure_scalar(erf_ctx *c) {
   if (c->sc_Q) return true;
-  double **arr[] = {&c->sc_Q, &c->sc_Qt, &c->sc_Qnew, &c->sc_sum[0], &c->sc_sum[1], &c->sc_sum[2], &c->sc_phi, &c->sc_R};
+  double **arr[] = {&c->sc_Q, &c->sc_Qt, &c->sc_Qnew, &c->sc_sum[0], &c->sc_sum[1], &c->sc_sum[2], &c->sc_phi, &c->sc_R,
+                    &c->sc_G[0], &c->sc_G[1]};
   for (auto p : arr) {
     *p = c->alloc(c->NW);
     if (!*p) return false;

@@ -632,3 +632,25 @@ def test_anelastic_mode_rejects_terrain_and_open_grids(torch, B):
         assert e.value.code == B.ERF_EUNSUPPORTED
         d.rk3_step(case["dt"], case["ns"])  # the context is still usable
         d.close()
+
+
+def test_scalar_on_the_fused_path_agrees_with_the_general_path(torch, B):
+    """With a scalar the flat periodic dycore stays on the fused kernels (the substep kernel accumulates the averaged
+    momenta, k_acoustic_flat<.., ACC>): far fewer launches than the all-general step, the same scalar and state."""
+    case = wl.make_case(5, nx=70, ny=24, nz=40)
+    rho0 = case["state"][0]
+    q0 = rho0 * (1.0 + 0.3 * np.random.default_rng(7).random(rho0.shape))
+    res = {}
+    for path in PATHS:
+        d = B.Dycore(case)
+        d.set_path(path)
+        d.set_state(*_dev(torch, case["state"]))
+        d.set_scalar(_dev(torch, [q0])[0])
+        n0 = d.launch_count
+        for _ in range(3):
+            d.rk3_step(case["dt"], case["ns"])
+        res[path] = (_host(d.get_state()), d.get_scalar().cpu().numpy(), d.launch_count - n0)
+        d.close()
+    assert res[0][2] < 0.5 * res[1][2], (res[0][2], res[1][2])
+    assert max(field_errors(res[0][0], res[1][0])) <= 3 * TOL_1STEP
+    assert np.abs(res[0][1] - res[1][1]).max() <= 3 * TOL_1STEP * np.abs(res[1][1]).max()
