@@ -114,6 +114,34 @@ inline void launch_columns(erf_ctx *c, cudaStream_t st, F f) {
   c->launches++;
 }
 
+// Per-cell passes as functors over the view type: CTAs whose 32 x 8 tile lies at least MARGIN columns inside the domain
+// run the body on a ViewNW (no wrap / clamp in the index helper), the others on the View.
+constexpr int MARGIN = 3;
+
+template <class F>
+__global__ void __launch_bounds__(256) k_cells_v(View v, int nlev, F f) {
+  // levels fastest in the launch order (vertical neighbours of the resident CTAs stay in L2)
+  const int i = blockIdx.y * 32 + threadIdx.x, j = blockIdx.z * 8 + threadIdx.y, k = blockIdx.x;
+  if (i >= v.nx || j >= v.ny || k >= nlev) return;
+  const int x0 = blockIdx.y * 32, y0 = blockIdx.z * 8;
+  const bool inner = x0 >= MARGIN && x0 + 32 + MARGIN <= v.nx && y0 >= MARGIN && y0 + 8 + MARGIN <= v.ny;
+  if (inner) {
+    const ViewNW vn(v);
+    f(vn, i, j, k);
+  } else {
+    f(v, i, j, k);
+  }
+}
+
+template <class F>
+inline void launch_cells_v(erf_ctx *c, cudaStream_t st, int nlev, const F &f) {
+  if (nlev <= 0) return;
+  dim3 block(32, 8), grid(nlev, (c->nx + 31) / 32, (c->ny + 7) / 8);
+  k_cells_v<<<grid, block, 0, st>>>(c->v, nlev, f);
+  c->launches++;
+}
+
+
 }  // namespace erfb
 
 namespace erfb {

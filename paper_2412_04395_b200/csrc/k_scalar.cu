@@ -21,100 +21,88 @@ namespace erfb {
 namespace {
 
 struct Sc {
-  View v;
   const double *rho, *U, *V, *W;     // stage state S^t
   const double *Us, *Vs, *Oms;       // sums over the substeps (null without substepping)
   double rn;                         // 1 / number of substeps
   bool folded;                       // the sums already hold n times the stage momenta (U, V, W are null)
+  bool diffuse;
   const double *Qt, *Qn, *K;
   double *phi, *Gx, *Gy, *R, *Qout;
   double dts;
 };
 
-__device__ __forceinline__ double mx(const Sc &s, int i, int j, int k) {  // averaged mass flux through x-face i
-  const size_t a = IX(s.v, i, j, k);
-  if (s.folded) return s.v.hx[a] * (s.rn * s.Us[a]);
-  return s.v.hx[a] * (s.U[a] + (s.Us ? s.rn * s.Us[a] : 0.0));
+template <class VT>
+__device__ __forceinline__ double mx(const VT &v, const Sc &s, int i, int j, int k) {  // averaged mass flux, x-face i
+  const size_t a = IX(v, i, j, k);
+  if (s.folded) return v.hx[a] * (s.rn * s.Us[a]);
+  return v.hx[a] * (s.U[a] + (s.Us ? s.rn * s.Us[a] : 0.0));
 }
-__device__ __forceinline__ double my(const Sc &s, int i, int j, int k) {
-  const size_t a = IX(s.v, i, j, k);
-  if (s.folded) return s.v.hy[a] * (s.rn * s.Vs[a]);
-  return s.v.hy[a] * (s.V[a] + (s.Vs ? s.rn * s.Vs[a] : 0.0));
+template <class VT>
+__device__ __forceinline__ double my(const VT &v, const Sc &s, int i, int j, int k) {
+  const size_t a = IX(v, i, j, k);
+  if (s.folded) return v.hy[a] * (s.rn * s.Vs[a]);
+  return v.hy[a] * (s.V[a] + (s.Vs ? s.rn * s.Vs[a] : 0.0));
 }
-__device__ __forceinline__ double mz(const Sc &s, int i, int j, int k) {  // averaged Omega through w-face k
-  if (k < 1 || k > s.v.nz - 1) return 0.0;
-  if (s.folded) return s.rn * s.Oms[IX(s.v, i, j, k)];  // flat grid: Omega = W
-  return gen::omega_at(s.v, s.U, s.V, s.W, i, j, k) + (s.Oms ? s.rn * s.Oms[IX(s.v, i, j, k)] : 0.0);
+template <class VT>
+__device__ __forceinline__ double mz(const VT &v, const Sc &s, int i, int j, int k) {  // averaged Omega, w-face k
+  if (k < 1 || k > v.nz - 1) return 0.0;
+  if (s.folded) return s.rn * s.Oms[IX(v, i, j, k)];  // flat grid: Omega = W
+  return gen::omega_at(v, s.U, s.V, s.W, i, j, k) + (s.Oms ? s.rn * s.Oms[IX(v, i, j, k)] : 0.0);
 }
 
 // mean vertical difference quotient of phi around level k at the two columns (ia, ja), (ib, jb): faces k and k+1
 // where they are interior (the chain-rule term of a horizontal derivative [R:G14])
-__device__ __forceinline__ double dz_mean(const Sc &s, int ia, int ja, int ib, int jb, int k) {
+template <class VT>
+__device__ __forceinline__ double dz_mean(const VT &v, const Sc &s, int ia, int ja, int ib, int jb, int k) {
   double sum = 0.0;
   int n = 0;
   for (int kk = k; kk <= k + 1; kk++)
-    if (kk >= 1 && kk <= s.v.nz - 1) {
-      const size_t a = IX(s.v, ia, ja, kk), b = IX(s.v, ib, jb, kk);
-      sum += (s.phi[a] - s.phi[IX(s.v, ia, ja, kk - 1)]) / s.v.hw[a] + (s.phi[b] - s.phi[IX(s.v, ib, jb, kk - 1)]) / s.v.hw[b];
+    if (kk >= 1 && kk <= v.nz - 1) {
+      const size_t a = IX(v, ia, ja, kk), b = IX(v, ib, jb, kk);
+      sum += (s.phi[a] - s.phi[IX(v, ia, ja, kk - 1)]) / v.hw[a] + (s.phi[b] - s.phi[IX(v, ib, jb, kk - 1)]) / v.hw[b];
       n += 2;
     }
   return n ? sum / n : 0.0;
 }
 
-__device__ __forceinline__ double gx_at(const Sc &s, int i, int j, int k) {  // diffusive flux through x-face i
-  const size_t a = IX(s.v, i, j, k), m = IX(s.v, i - 1, j, k);
-  const double d = (s.phi[a] - s.phi[m]) / s.v.dx - s.v.sxu[a] * dz_mean(s, i - 1, j, i, j, k);
-  return -0.5 * (s.K[m] + s.K[a]) * d;
-}
-__device__ __forceinline__ double gy_at(const Sc &s, int i, int j, int k) {
-  const size_t a = IX(s.v, i, j, k), m = IX(s.v, i, j - 1, k);
-  const double d = (s.phi[a] - s.phi[m]) / s.v.dy - s.v.syv[a] * dz_mean(s, i, j - 1, i, j, k);
-  return -0.5 * (s.K[m] + s.K[a]) * d;
-}
-
-}  // namespace
-
-// Q_stage from Q^t (stage value) and Q^n; nsub = 0: no substepping (the stage momenta advect)
-void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, double *Qout, int nsub, double dts,
-                  cudaStream_t st, bool folded) {
+struct FPhi {
   Sc s;
-  s.v = c->v;
-  s.folded = folded;
-  s.rho = St.f[RHO]; s.U = St.f[UU]; s.V = St.f[VV]; s.W = St.f[WW];
-  s.Us = nsub ? c->sc_sum[0] : nullptr; s.Vs = nsub ? c->sc_sum[1] : nullptr; s.Oms = nsub ? c->sc_sum[2] : nullptr;
-  s.rn = nsub ? 1.0 / nsub : 0.0;
-  s.Qt = Qt; s.Qn = Qn; s.K = c->p.diffusion != 0 ? (folded ? c->fz->Kd : c->diff.K) : nullptr;
-  s.phi = c->sc_phi; s.R = c->sc_R; s.Qout = Qout;
-  s.Gx = folded ? c->sc_G[0] : c->diff.Fx; s.Gy = folded ? c->sc_G[1] : c->diff.Fy;
-  s.dts = dts;
-  const int nz = c->nz;
-  const bool diffuse = c->p.diffusion != 0;
-  if (!folded)
-    launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
-      const size_t a = IX(s.v, i, j, k);
-      s.phi[a] = s.Qt[a] / s.rho[a];
-    });
-  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
-    const View &v = s.v;
+  template <class VT> __device__ void operator()(const VT &v, int i, int j, int k) const {
     const size_t a = IX(v, i, j, k);
-    const double fxm = mx(s, i, j, k), fxp = mx(s, i + 1, j, k), fym = my(s, i, j, k), fyp = my(s, i, j + 1, k);
-    const double omm = mz(s, i, j, k), omp = mz(s, i, j, k + 1);
+    s.phi[a] = s.Qt[a] / s.rho[a];
+  }
+};
+
+struct FAdvect {
+  Sc s;
+  template <class VT> __device__ void operator()(const VT &v, int i, int j, int k) const {
+    const size_t a = IX(v, i, j, k);
+    const double fxm = mx(v, s, i, j, k), fxp = mx(v, s, i + 1, j, k), fym = my(v, s, i, j, k), fyp = my(v, s, i, j + 1, k);
+    const double omm = mz(v, s, i, j, k), omp = mz(v, s, i, j, k + 1);
     const double ax = fxp * gen::interp_x(v, s.phi, i + 1, j, k, v.osh, fxp) - fxm * gen::interp_x(v, s.phi, i, j, k, v.osh, fxm);
     const double ay = fyp * gen::interp_y(v, s.phi, i, j + 1, k, v.osh, fyp) - fym * gen::interp_y(v, s.phi, i, j, k, v.osh, fym);
     const double zt = (k + 1 <= v.nz - 1) ? omp * gen::interp_z(v, s.phi, i, j, k + 1, 0, v.nz - 1, v.osv, omp) : 0.0;
     const double zb = (k >= 1) ? omm * gen::interp_z(v, s.phi, i, j, k, 0, v.nz - 1, v.osv, omm) : 0.0;
     const double R = -(ax / v.dx + ay / v.dy + (zt - zb)) / v.hc[a];
-    if (diffuse) s.R[a] = R;
+    if (s.diffuse) s.R[a] = R;
     else s.Qout[a] = s.Qn[a] + s.dts * R;
-  });
-  if (!diffuse) return;
-  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
-    const size_t a = IX(s.v, i, j, k);
-    s.Gx[a] = gx_at(s, i, j, k);
-    s.Gy[a] = gy_at(s, i, j, k);
-  });
-  launch_cells(c, st, nz, [=] __device__(int i, int j, int k) {
-    const View &v = s.v;
+  }
+};
+
+struct FHFlux {  // diffusive fluxes through the x- and y-faces
+  Sc s;
+  template <class VT> __device__ void operator()(const VT &v, int i, int j, int k) const {
+    const size_t a = IX(v, i, j, k), mxi = IX(v, i - 1, j, k), myi = IX(v, i, j - 1, k);
+    const double dxp = (s.phi[a] - s.phi[mxi]) / v.dx - v.sxu[a] * dz_mean(v, s, i - 1, j, i, j, k);
+    const double dyp = (s.phi[a] - s.phi[myi]) / v.dy - v.syv[a] * dz_mean(v, s, i, j - 1, i, j, k);
+    s.Gx[a] = -0.5 * (s.K[mxi] + s.K[a]) * dxp;
+    s.Gy[a] = -0.5 * (s.K[myi] + s.K[a]) * dyp;
+  }
+};
+
+struct FDiffuse {
+  Sc s;
+  template <class VT> __device__ void operator()(const VT &v, int i, int j, int k) const {
     const size_t a = IX(v, i, j, k), ip = IX(v, i + 1, j, k), jp = IX(v, i, j + 1, k);
     // contravariant vertical flux through w-face kk (zero on the lids)
     auto gz = [&](int kk) -> double {
@@ -128,7 +116,30 @@ void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, 
     const double div = ((v.hx[ip] * s.Gx[ip] - v.hx[a] * s.Gx[a]) / v.dx + (v.hy[jp] * s.Gy[jp] - v.hy[a] * s.Gy[a]) / v.dy +
                         (gz(k + 1) - gz(k))) / v.hc[a];
     s.Qout[a] = s.Qn[a] + s.dts * (s.R[a] - div);
-  });
+  }
+};
+
+}  // namespace
+
+// Q_stage from Q^t (stage value) and Q^n; nsub = 0: no substepping (the stage momenta advect)
+void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, double *Qout, int nsub, double dts,
+                  cudaStream_t st, bool folded) {
+  Sc s;
+  s.folded = folded;
+  s.rho = St.f[RHO]; s.U = St.f[UU]; s.V = St.f[VV]; s.W = St.f[WW];
+  s.Us = nsub ? c->sc_sum[0] : nullptr; s.Vs = nsub ? c->sc_sum[1] : nullptr; s.Oms = nsub ? c->sc_sum[2] : nullptr;
+  s.rn = nsub ? 1.0 / nsub : 0.0;
+  s.Qt = Qt; s.Qn = Qn; s.K = c->p.diffusion != 0 ? (folded ? c->fz->Kd : c->diff.K) : nullptr;
+  s.phi = c->sc_phi; s.R = c->sc_R; s.Qout = Qout;
+  s.Gx = folded ? c->sc_G[0] : c->diff.Fx; s.Gy = folded ? c->sc_G[1] : c->diff.Fy;
+  s.dts = dts;
+  s.diffuse = c->p.diffusion != 0;
+  const int nz = c->nz;
+  if (!folded) launch_cells_v(c, st, nz, FPhi{s});
+  launch_cells_v(c, st, nz, FAdvect{s});
+  if (!s.diffuse) return;
+  launch_cells_v(c, st, nz, FHFlux{s});
+  launch_cells_v(c, st, nz, FDiffuse{s});
 }
 
 // fused flat path, before the substeps of a stage: phi^t = Q^t / rho^t and the sums started at n times the stage momenta
