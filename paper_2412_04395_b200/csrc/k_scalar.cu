@@ -15,6 +15,7 @@
 // the stage state, so there the sums are started at n times the stage momenta ("folded") and phi^t is formed before the
 // substeps (scalar_prepare_fused); the stage then needs nothing of S^t.
 #include "fused.cuh"
+#include "slow_flat.cuh"
 
 namespace erfb {
 
@@ -89,12 +90,47 @@ struct FAdvect {
   }
 };
 
+// The same advective tendency with a compile-time horizontal order, the lateral offsets wrapped / clamped once per
+// thread and flux = M q_even - |M| q_odd (as tslow::k_adv_terrain does for theta); Eq. 17-21 only.
+template <int OH>
+__global__ void __launch_bounds__(256) k_scalar_adv(View v, Sc s) {
+  const int i = blockIdx.y * 32 + threadIdx.x, j = blockIdx.z * 8 + threadIdx.y, k = blockIdx.x;
+  const int nx = v.nx, ny = v.ny, nz = v.nz;
+  if (i >= nx || j >= ny) return;
+  const size_t plane = (size_t)nx * ny, kb = (size_t)k * plane;
+  int xo[7];
+  size_t yo[7];
+#pragma unroll
+  for (int n = 0; n < 7; n++) {
+    xo[n] = lati(i + n - 3, nx, v.perx);
+    yo[n] = (size_t)lati(j + n - 3, ny, v.pery) * nx;
+  }
+  const size_t oc = yo[3] + xo[3], a = kb + oc;
+  const double fxm = mx(v, s, i, j, k), fxp = mx(v, s, i + 1, j, k), fym = my(v, s, i, j, k), fyp = my(v, s, i, j + 1, k);
+  const double omm = mz(v, s, i, j, k), omp = mz(v, s, i, j, k + 1);
+  double q[7];
+#pragma unroll
+  for (int n = 0; n < 7; n++) q[n] = s.phi[kb + yo[3] + xo[n]];
+  double acc = (flux_c<OH>(fxp, q[1], q[2], q[3], q[4], q[5], q[6]) - flux_c<OH>(fxm, q[0], q[1], q[2], q[3], q[4], q[5])) / v.dx;
+#pragma unroll
+  for (int n = 0; n < 7; n++) q[n] = s.phi[kb + yo[n] + xo[3]];
+  acc += (flux_c<OH>(fyp, q[1], q[2], q[3], q[4], q[5], q[6]) - flux_c<OH>(fym, q[0], q[1], q[2], q[3], q[4], q[5])) / v.dy;
+#pragma unroll
+  for (int n = 0; n < 7; n++) q[n] = s.phi[(size_t)min(max(k + n - 3, 0), nz - 1) * plane + oc];
+  const double zt = (k + 1 <= nz - 1) ? flux_rt(vorder(v.ov, min(k + 1, nz - k - 1)), omp, q + 1) : 0.0;
+  const double zb = (k >= 1) ? flux_rt(vorder(v.ov, min(k, nz - k)), omm, q) : 0.0;
+  const double R = -(acc + (zt - zb)) / v.hc[a];
+  if (s.diffuse) s.R[a] = R;
+  else s.Qout[a] = s.Qn[a] + s.dts * R;
+}
+
 struct FHFlux {  // diffusive fluxes through the x- and y-faces
   Sc s;
   template <class VT> __device__ void operator()(const VT &v, int i, int j, int k) const {
     const size_t a = IX(v, i, j, k), mxi = IX(v, i - 1, j, k), myi = IX(v, i, j - 1, k);
-    const double dxp = (s.phi[a] - s.phi[mxi]) / v.dx - v.sxu[a] * dz_mean(v, s, i - 1, j, i, j, k);
-    const double dyp = (s.phi[a] - s.phi[myi]) / v.dy - v.syv[a] * dz_mean(v, s, i, j - 1, i, j, k);
+    // (on a flat grid the slopes vanish identically: the chain-rule terms are skipped, not multiplied by zero)
+    const double dxp = (s.phi[a] - s.phi[mxi]) / v.dx - (v.flat ? 0.0 : v.sxu[a] * dz_mean(v, s, i - 1, j, i, j, k));
+    const double dyp = (s.phi[a] - s.phi[myi]) / v.dy - (v.flat ? 0.0 : v.syv[a] * dz_mean(v, s, i, j - 1, i, j, k));
     s.Gx[a] = -0.5 * (s.K[mxi] + s.K[a]) * dxp;
     s.Gy[a] = -0.5 * (s.K[myi] + s.K[a]) * dyp;
   }
@@ -109,6 +145,7 @@ struct FDiffuse {
       if (kk < 1 || kk > v.nz - 1) return 0.0;
       const size_t f = IX(v, i, j, kk), b = IX(v, i, j, kk - 1);
       const double fz = -0.5 * (s.K[b] + s.K[f]) * ((s.phi[f] - s.phi[b]) / v.hw[f]);
+      if (v.flat) return fz;
       const double gxb = 0.25 * (s.Gx[b] + s.Gx[IX(v, i + 1, j, kk - 1)] + s.Gx[f] + s.Gx[IX(v, i + 1, j, kk)]);
       const double gyb = 0.25 * (s.Gy[b] + s.Gy[IX(v, i, j + 1, kk - 1)] + s.Gy[f] + s.Gy[IX(v, i, j + 1, kk)]);
       return fz - v.sxw[f] * gxb - v.syw[f] * gyb;
@@ -136,7 +173,19 @@ void scalar_stage(erf_ctx *c, const F5 &St, const double *Qt, const double *Qn, 
   s.diffuse = c->p.diffusion != 0;
   const int nz = c->nz;
   if (!folded) launch_cells_v(c, st, nz, FPhi{s});
-  launch_cells_v(c, st, nz, FAdvect{s});
+  if (c->v.osh == c->v.oh && c->v.osv == c->v.ov) {
+    dim3 block(32, 8), grid(nz, (c->nx + 31) / 32, (c->ny + 7) / 8);
+    switch (c->v.oh) {
+      case 2: k_scalar_adv<2><<<grid, block, 0, st>>>(c->v, s); break;
+      case 3: k_scalar_adv<3><<<grid, block, 0, st>>>(c->v, s); break;
+      case 4: k_scalar_adv<4><<<grid, block, 0, st>>>(c->v, s); break;
+      case 5: k_scalar_adv<5><<<grid, block, 0, st>>>(c->v, s); break;
+      default: k_scalar_adv<6><<<grid, block, 0, st>>>(c->v, s); break;
+    }
+    c->launches++;
+  } else {
+    launch_cells_v(c, st, nz, FAdvect{s});  // WENO (L213)
+  }
   if (!s.diffuse) return;
   launch_cells_v(c, st, nz, FHFlux{s});
   launch_cells_v(c, st, nz, FDiffuse{s});
