@@ -573,7 +573,8 @@ def _numpy_divergence(case, st):
 @pytest.mark.parametrize("cfg,kw,stretch", [(1, dict(nx=40, ny=23, nz=19), 1.0), (3, dict(nx=46, ny=21, nz=34), 1.06),
                                             (2, dict(nx=32, ny=16, nz=21), 1.0), (5, dict(nx=70, ny=11, nz=40), 1.03),
                                             (3, dict(nx=64, ny=128, nz=12), 1.0), (1, dict(nx=2, ny=4, nz=6), 1.0),
-                                            (2, dict(nx=40, ny=32, nz=9), 1.0)])
+                                            (2, dict(nx=40, ny=32, nz=9), 1.0), (1, dict(nx=5, ny=1, nz=7), 1.0),
+                                            (1, dict(nx=1, ny=1, nz=4), 1.0), (1, dict(nx=6, ny=8, nz=1), 1.0)])
 def test_anelastic_mode_matches_oracle(torch, erfo, B, cfg, kw, stretch):
     """The projection alone (Eq. 16) on momenta that are far from divergence-free, then three RK2 steps (Eq. 14-15) of a
     warm bubble in the configuration's wind, against the oracle: state, lagged p', and div(rho0 u) = 0 on the device
@@ -620,7 +621,8 @@ def test_anelastic_mode_matches_oracle(torch, erfo, B, cfg, kw, stretch):
     assert np.abs(pgot - pref).max() <= 1e-9 * np.abs(pref).max()
     assert np.abs(_numpy_divergence(case, got)).max() <= 1e-11 * div0
     assert np.array_equal(got[0], rho0)
-    assert np.abs(got[4] - st[4]).max() > 1e-6 * np.abs(st[4]).max()      # the bubble moved
+    if nx * ny > 1 and nz > 1:
+        assert np.abs(got[4] - st[4]).max() > 1e-6 * np.abs(st[4]).max()  # the bubble moved
 
 
 def test_anelastic_mode_rejects_terrain_and_open_grids(torch, B):
