@@ -19,15 +19,19 @@
  * and of the scalar diffusion flux on single Fourier / cosine modes (Eq. 2-3,
  * Eq. 9), mu = rho*nu with edge means, K = mu_t/Pr_t, the divergence-damping
  * recurrence (L144), kinematic lids over terrain, chain-rule metric terms of
- * the strain and of the scalar flux on Cartesian-linear fields.
+ * the strain and of the scalar flux on Cartesian-linear fields;
+ * test_oracle_scalar.py (Eq. 4 with the averaged momenta), test_oracle_weno.py
+ * (WENO-JS / WENO-Z from their definitions), test_oracle_open_rayleigh.py
+ * (open and inflow boundaries, Rayleigh layer), test_oracle_anelastic.py
+ * (Eq. 8, 14-16: dense brute-force projection, invariants, RK2 polynomial).
  * The full nonlinear step on the benchmark configurations has no value
  * printed in the paper: "parity unpinned" beyond those invariants.
  *
  * Notation.  Cells (i,j,k), x fastest.  State S = (rho, U, V, W, Theta),
  * Theta = rho*theta.  U on x-faces (i-1/2,j,k), V on y-faces, W on z-faces
- * k = 0..nz.  Periodic in x and y; rigid free-slip lids at k = 0 and k = nz.
- * Work arrays carry NG ghost cells in x and y, filled periodically after
- * every field is computed.
+ * k = 0..nz.  Laterally periodic, open or inflow/outflow per direction; rigid
+ * free-slip lids at k = 0 and k = nz.  Work arrays carry NG ghost cells in x
+ * and y, filled by the lateral boundary rule after every field is computed.
  */
 #include "erf_oracle.h"
 
