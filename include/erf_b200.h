@@ -51,8 +51,9 @@ typedef struct {
                                  every ghost value is the nearest interior value (zero normal gradient,
                                  DESIGN.md reading G27); 2 inflow at the low side, open (outflow) at the high
                                  side: the first column of cells -- rho*u on the boundary face included -- is
-                                 held at the values given to erf_set_state (reading G30); non-periodic grids
-                                 run the terrain-general kernels                                           */
+                                 held at the values given to erf_set_state (reading G30; the five prognostic
+                                 fields only: a transported scalar sees the open closure there); non-periodic
+                                 grids run the terrain-general kernels                                     */
 } erf_grid;
 
 typedef struct {
