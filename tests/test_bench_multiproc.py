@@ -64,3 +64,21 @@ def test_reference_arm_under_torchrun_prints_one_line():
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_algorithmic_bytes_and_committed_traffic():
+    """B_alg per cell-step = 2128 B (configs 1, 2), 2176 B (3, 5), 3040 B (4); and the ncu traffic file that
+    bench.py's roofline.traffic reads carries both kernel classes, above their algorithmic bytes."""
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2412_04395_b200 import workloads as wl
+    want = {1: 2128, 2: 2128, 3: 2176, 4: 3040, 5: 2176}
+    for cfg, b in want.items():
+        case = wl.make_case(cfg, nx=8, ny=8, with_state=False)
+        assert bench.algorithmic_doubles(case)["total"] * 8 == b, cfg
+    cells = 1024 * 1024 * 128
+    ac, sl = bench.measured_traffic("acoustic_fused", 5), bench.measured_traffic("slow_rhs_fused", 5)
+    assert ac is not None and sl is not None
+    assert 20 * 8 * cells < ac < 2.0 * 20 * 8 * cells
+    assert 14 * 8 * cells < sl < 4.0 * 14 * 8 * cells
+    assert bench.measured_traffic("acoustic_fused", 3) is None
