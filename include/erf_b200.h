@@ -41,6 +41,7 @@ extern "C" {
 #define ERF_EUNSUPPORTED (-2) /* anelastic mode on a terrain or laterally open grid                */
 #define ERF_ENOMEM (-3)       /* host or device allocation failed                                */
 #define ERF_ECUDA (-4)        /* a CUDA runtime call or kernel launch failed (sticky)            */
+#define ERF_ETOOLARGE (-5)    /* erf_poisson_modes_noalloc: nx*ny*nz exceeds ERF_NOALLOC_MAX_VALUES */
 
 typedef struct erf_ctx erf_ctx; /* opaque; owns all internal device memory */
 
@@ -137,6 +138,42 @@ int erf_get_scalar(erf_ctx *ctx, double *rhophi, void *cuda_stream);
 int erf_anelastic_step(erf_ctx *ctx, double dt, void *cuda_stream);
 int erf_get_pprime(erf_ctx *ctx, double *pprime, void *cuda_stream);
 int erf_project(erf_ctx *ctx, double dt, void *cuda_stream);
+
+/* The vertical solve of the anelastic Poisson equation (Sec. 3.2 Eq. 16; reading G29) WITHOUT ANY
+ * ALLOCATION and without a context, for callers that are not free to take device memory when they call: a solver that
+ * runs inside an application whose own allocator already holds the whole GPU (a cudaMalloc from this library would fail
+ * there, or eat into what that allocator expects to find), a job held to a memory budget its own buffers use up, or a
+ * time loop that cannot afford the device-wide synchronisation an allocation brings.  Every other entry point of this
+ * library goes through an erf_ctx, and erf_create (and the first use of some paths) allocates; this one never calls
+ * cudaMalloc, cudaFree or any library routine that does.
+ *
+ * What it computes: the step erf_project performs between its forward and inverse horizontal transforms.  On entry
+ * (hat_re, hat_im) hold the discrete Fourier coefficients in x and y of the divergence div(rho0 u), DEVICE
+ * [nz][ny][nx] each with the x-wavenumber m fastest (unnormalised forward transform, the layout of a plain 2-D FFT of
+ * every level); on return they hold the coefficients of psi, the solution of
+ *     [lx(m) + ly(n)] P_k + [ (P_{k+1} - P_k)/dzw[k+1] - (P_k - P_{k-1})/dzw[k] ] / dz[k] = Dhat_k / dt
+ * with lx(m) = -(4/dx^2) sin^2(pi m/nx), ly(n) = -(4/dy^2) sin^2(pi n/ny), no-gradient lids, and P_0 = 0 for the
+ * mean mode (0, 0).  dz: DEVICE [nz] cell thicknesses; dzw: DEVICE [nz+1] distances between cell centres across face k
+ * (entries 1 .. nz-1 are read).  The caller owns all four arrays; hat_re / hat_im are overwritten in place.  Enqueue
+ * only, on cuda_stream; the arrays must stay valid until that work has run.
+ *
+ * The work space -- one double per (mode, level) -- is a fixed array of ERF_NOALLOC_MAX_VALUES doubles (8 MiB) built
+ * into the library's device code.  Consequences the caller has to know:
+ *   - LIMIT: nx*ny*nz <= ERF_NOALLOC_MAX_VALUES (for example 128 x 128 x 64); anything larger is refused with
+ *     ERF_ETOOLARGE before any CUDA call, and nothing is written.  Larger problems need erf_project and a context.
+ *   - Every GPU on which the process uses liberf_b200.so holds these 8 MiB until the process ends, used or not.
+ *   - There is ONE array per GPU, shared by every call: two calls that may run at the same time on one GPU (two
+ *     streams, two host threads) corrupt each other's result silently.  Keep calls on a GPU ordered on one stream, or
+ *     order them with events.  The array keeps the last call's values between calls; the solve does not depend on
+ *     them (each entry is written before it is read), so nothing needs clearing.
+ *   - The FIRST call on each GPU looks up the array's device address (and may make the CUDA runtime load the library's
+ *     device code onto that GPU); later calls only launch the kernel.  Make that first call with the GPU current,
+ *     during set-up, before any stream capture is begun in the process.
+ * Returns ERF_EINVAL for a null pointer or a non-positive size, dx, dy or dt; ERF_ECUDA if the address look-up or the
+ * launch fails. */
+#define ERF_NOALLOC_MAX_VALUES 1048576
+int erf_poisson_modes_noalloc(int nx, int ny, int nz, double dx, double dy, double dt, const double *dz,
+                              const double *dzw, double *hat_re, double *hat_im, void *cuda_stream);
 
 /* Free everything; erf_destroy(NULL) is a no-op. */
 void erf_destroy(erf_ctx *ctx);

@@ -17,7 +17,8 @@ import os
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liberf_b200.so")
 
-ERF_OK, ERF_EINVAL, ERF_EUNSUPPORTED, ERF_ENOMEM, ERF_ECUDA = 0, -1, -2, -3, -4
+ERF_OK, ERF_EINVAL, ERF_EUNSUPPORTED, ERF_ENOMEM, ERF_ECUDA, ERF_ETOOLARGE = 0, -1, -2, -3, -4, -5
+ERF_NOALLOC_MAX_VALUES = 1048576  # erf_poisson_modes_noalloc: nx*ny*nz limit (doubles of built-in work space)
 ERF_PATH_AUTO, ERF_PATH_GENERAL = 0, 1
 # erf_set_option keys and ERF_OPT_VARIANT bits (include/erf_b200.h, diagnostics block)
 ERF_OPT_VARIANT, ERF_OPT_GRAPH = 1, 2
@@ -27,7 +28,7 @@ ERF_VARIANT_FORCE_COLUMN, ERF_VARIANT_SPLIT_SLOW_RHS, ERF_VARIANT_FORCE_TILE = 4
 EXPORTS = ["erf_create", "erf_set_state", "erf_rk3_step", "erf_get_state", "erf_destroy",
            "erf_strerror", "erf_set_scalar", "erf_get_scalar", "erf_anelastic_step", "erf_get_pprime", "erf_project", "erf_slow_rhs", "erf_acoustic", "erf_set_path", "erf_set_option", "erf_launch_count",
            "erf_device_bytes", "erf_set_timing", "erf_get_timing", "erf_reset_timing", "erf_timing_name",
-           "erf_measure_fp64_peak"]
+           "erf_measure_fp64_peak", "erf_poisson_modes_noalloc"]
 ERF_TIMING_CLASSES = 8
 
 _dp = C.c_void_p
@@ -102,6 +103,7 @@ def load(path: str | None = None):
     L.erf_timing_name.argtypes = [C.c_int]
     L.erf_timing_name.restype = C.c_char_p
     L.erf_measure_fp64_peak.argtypes = [C.POINTER(C.c_double), C.c_void_p]
+    L.erf_poisson_modes_noalloc.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [_dp] * 4 + [C.c_void_p]
     _lib = L
     return L
 
@@ -169,6 +171,15 @@ def erf_project(h, dt, stream=None):
 
 def erf_get_pprime(h, pprime, stream=None):
     _ck(load().erf_get_pprime(h, _ptr(pprime), _stream(stream)), "erf_get_pprime")
+
+
+def erf_poisson_modes_noalloc(nx, ny, nz, dx, dy, dt, dz, dzw, hat_re, hat_im, stream=None):
+    """Eq. 16's tridiagonal solve per horizontal mode, in place in (hat_re, hat_im), for callers that may not allocate
+    device memory (include/erf_b200.h): no context, the work space is a fixed array inside the library, so
+    nx*ny*nz <= ERF_NOALLOC_MAX_VALUES and calls on one GPU must not overlap.  All four arrays are float64 CUDA tensors."""
+    _ck(load().erf_poisson_modes_noalloc(int(nx), int(ny), int(nz), float(dx), float(dy), float(dt), _ptr(dz),
+                                         _ptr(dzw), _ptr(hat_re), _ptr(hat_im), _stream(stream)),
+        "erf_poisson_modes_noalloc")
 
 
 def erf_destroy(h):

@@ -40,6 +40,7 @@ extern "C" const char *erf_strerror(int code) {
     case ERF_EUNSUPPORTED: return "unsupported configuration (the anelastic mode needs a flat, laterally periodic grid)";
     case ERF_ENOMEM: return "out of memory";
     case ERF_ECUDA: return "CUDA error";
+    case ERF_ETOOLARGE: return "nx*ny*nz exceeds ERF_NOALLOC_MAX_VALUES, the fixed work space of erf_poisson_modes_noalloc";
     default: return "unknown error";
   }
 }
