@@ -3,6 +3,7 @@
 #include <cstring>
 
 #include "acoustic_args.cuh"
+#include "slow_flat.cuh"
 
 namespace erfb {
 
@@ -110,7 +111,9 @@ int fused_setup(erf_ctx *c, const erf_metrics *m, cudaStream_t st) {
     if (!z->mu || !z->Kd) return c->status;
     if (!ensure_prim(c, false)) return c->status;  // u, v, w for the diffusion kernels
   }
-  if ((c->nx & 1) && !ensure_prim(c, false)) return c->status;  // odd nx: the round-1 slow-RHS kernels
+  // wherever the round-1 slow-RHS kernels run instead of k_slow_adv (odd nx, nz + 1 beyond its level tables): k_prim_flat
+  // writes u, v, w, p' whether or not diffusion reads them
+  if (!slow_adv_available(c) && !ensure_prim(c, false)) return c->status;
   return ERF_OK;
 }
 

@@ -403,6 +403,31 @@ def test_round1_slow_rhs_kernels_agree_with_the_fused_one(torch, erfo, B, cfg, k
     assert max(field_errors(old, ref)) <= 2 * TOL_1STEP, field_errors(old, ref)
 
 
+@pytest.mark.parametrize("cfg,kw", [(3, dict(nx=8, ny=6, nz=320, params=dict(diffusion=0))), (3, dict(nx=8, ny=6, nz=321)),
+                                    (5, dict(nx=34, ny=5, nz=330, params=dict(diffusion=0)))])
+def test_more_levels_than_the_fused_slow_rhs_tables_hold(torch, erfo, B, cfg, kw):
+    """nz + 1 > 320 is beyond k_slow_adv's shared-memory level tables: the context falls back to the round-1 slow-RHS
+    kernels, which write u, v, w and p' -- arrays that used to be allocated only with diffusion on or odd nx, so that a
+    deep even-nx grid without diffusion wrote through null pointers.  One slow right-hand side
+    and two full steps against the oracle, without and with diffusion."""
+    case = wl.make_case(cfg, **kw)
+    assert case["nz"] + 1 > 320 and case["nx"] % 2 == 0
+    o = erfo.Oracle(case)
+    o.set_state(*case["state"])
+    ref = o.slow_rhs()
+    o.close()
+    d = B.Dycore(case)
+    d.set_state(*_dev(torch, case["state"]))
+    got = _host(d.slow_rhs())
+    d.close()
+    for f, (a, b) in enumerate(zip(got, ref)):
+        scale = max(np.abs(b).max(), 1e-300)
+        assert np.abs(a - b).max() / scale <= TOL_RHS, (f, np.abs(a - b).max() / scale)
+    ref = _run_oracle(erfo, case, 2)
+    got = _run_gpu(torch, B, case, 2)
+    assert max(field_errors(got, ref)) <= 2 * TOL_1STEP, field_errors(got, ref)
+
+
 @pytest.mark.parametrize("cfg,kw", [(1, dict()), (2, dict(nx=64, ny=48, nz=32))])
 def test_cuda_graph_replay_is_bitwise_the_stream_launch(torch, B, cfg, kw):
     """ERF_OPT_GRAPH: the step replayed from captured CUDA graphs (one per buffer configuration) must give the very
@@ -411,6 +436,29 @@ def test_cuda_graph_replay_is_bitwise_the_stream_launch(torch, B, cfg, kw):
     a = _run_gpu(torch, B, case, 9)
     b = _run_gpu(torch, B, case, 9, graph=True)
     for x, y in zip(a, b):
+        assert np.array_equal(x, y)
+
+
+def test_cuda_graph_cache_survives_a_changing_time_step(torch, B):
+    """A caller whose dt changes from step to step (more distinct values than the graph cache keeps, so the least
+    recently used graphs are destroyed and captured again) gets the bits of plain stream launches."""
+    case = wl.make_case(2, nx=64, ny=48, nz=32)
+    dts = [case["dt"] * f for f in (1.0, 0.9, 0.8, 0.7, 0.6, 0.5, 1.0, 0.9, 0.55, 1.0, 1.0, 0.8)] * 2
+    res = []
+    for graph in (False, True):
+        d = B.Dycore(case)
+        if graph:
+            d.set_option(B.ERF_OPT_GRAPH, 1)
+        d.set_state(*_dev(torch, case["state"]))
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            for dt in dts:
+                d.rk3_step(dt, case["ns"])
+        side.synchronize()
+        res.append(_host(d.get_state()))
+        d.close()
+    for x, y in zip(*res):
         assert np.array_equal(x, y)
 
 
@@ -634,6 +682,21 @@ def test_anelastic_mode_rejects_terrain_and_open_grids(torch, B):
         assert e.value.code == B.ERF_EUNSUPPORTED
         d.rk3_step(case["dt"], case["ns"])  # the context is still usable
         d.close()
+    # a transported scalar has no stage in the RK2 step: refused, not silently left behind
+    case = wl.make_case(1, nx=16, ny=16, nz=8)
+    d = B.Dycore(case)
+    st = _dev(torch, case["state"])
+    d.set_state(*st)
+    d.anelastic_step(0.5)
+    d.set_scalar(st[0].clone())
+    before = _host(d.get_state())
+    with pytest.raises(B.ErfError) as e:
+        d.anelastic_step(0.5)
+    assert e.value.code == B.ERF_EUNSUPPORTED
+    assert all(np.array_equal(a, b) for a, b in zip(before, _host(d.get_state())))
+    d.project(0.5)
+    d.rk3_step(case["dt"], case["ns"])
+    d.close()
 
 
 def test_scalar_on_the_fused_path_agrees_with_the_general_path(torch, B):
@@ -653,6 +716,6 @@ def test_scalar_on_the_fused_path_agrees_with_the_general_path(torch, B):
             d.rk3_step(case["dt"], case["ns"])
         res[path] = (_host(d.get_state()), d.get_scalar().cpu().numpy(), d.launch_count - n0)
         d.close()
-    assert res[0][2] < 0.5 * res[1][2], (res[0][2], res[1][2])
+    assert res[0][2] < 0.5 * res[1][2], (res[0][2], res[1][2])  # kernel launch counts (erf_launch_count), not times
     assert max(field_errors(res[0][0], res[1][0])) <= 3 * TOL_1STEP
     assert np.abs(res[0][1] - res[1][1]).max() <= 3 * TOL_1STEP * np.abs(res[1][1]).max()
