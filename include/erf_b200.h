@@ -38,7 +38,7 @@ extern "C" {
 
 #define ERF_OK 0
 #define ERF_EINVAL (-1)       /* null pointer, non-positive size, bad order / substep count / dt / option */
-#define ERF_EUNSUPPORTED (-2) /* anelastic mode on a terrain or laterally open grid                */
+#define ERF_EUNSUPPORTED (-2) /* anelastic mode on a terrain or laterally open grid, or with a scalar */
 #define ERF_ENOMEM (-3)       /* host or device allocation failed                                */
 #define ERF_ECUDA (-4)        /* a CUDA runtime call or kernel launch failed (sticky)            */
 #define ERF_ETOOLARGE (-5)    /* erf_poisson_modes_noalloc: nx*ny*nz exceeds ERF_NOALLOC_MAX_VALUES */
@@ -133,6 +133,8 @@ int erf_get_scalar(erf_ctx *ctx, double *rhophi, void *cuda_stream);
  * (L94).  The Poisson equation is solved by a discrete Fourier transform in x and y and a tridiagonal system in z per
  * mode (reading G29), so the grid must be flat and periodic in x and y: otherwise ERF_EUNSUPPORTED.
  * Uses the same context, state and parameters as erf_rk3_step; p' starts at zero and lives in the context.
+ * A transported scalar (erf_set_scalar) is advanced by erf_rk3_step only: on a context that has one,
+ * erf_anelastic_step returns ERF_EUNSUPPORTED and changes nothing (erf_project still works).
  * erf_get_pprime: DEVICE [nz][ny][nx]; ERF_EINVAL before the first anelastic call.
  * erf_project applies the projection alone to the momenta of the current state (tests). */
 int erf_anelastic_step(erf_ctx *ctx, double dt, void *cuda_stream);

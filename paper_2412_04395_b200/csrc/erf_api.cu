@@ -3,6 +3,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <utility>
 
 #include "erf_ctx.cuh"
 #include "fused.cuh"
@@ -26,6 +27,14 @@ double *erf_ctx::alloc(size_t n) {
   return (double *)p;
 }
 
+// a copy with its own return code checked: a bad caller pointer is reported by the call that was given it
+static void copy(erf_ctx *c, void *dst, const void *src, size_t bytes, cudaMemcpyKind kind, cudaStream_t st) {
+  if (cudaMemcpyAsync(dst, src, bytes, kind, st) != cudaSuccess) {
+    cudaGetLastError();
+    c->status = ERF_ECUDA;
+  }
+}
+
 static int check(erf_ctx *c) {
   if (c->status != ERF_OK) return c->status;
   cudaError_t e = cudaGetLastError();
@@ -37,7 +46,7 @@ extern "C" const char *erf_strerror(int code) {
   switch (code) {
     case ERF_OK: return "ok";
     case ERF_EINVAL: return "invalid argument";
-    case ERF_EUNSUPPORTED: return "unsupported configuration (the anelastic mode needs a flat, laterally periodic grid)";
+    case ERF_EUNSUPPORTED: return "unsupported configuration (the anelastic mode needs a flat, laterally periodic grid and no transported scalar)";
     case ERF_ENOMEM: return "out of memory";
     case ERF_ECUDA: return "CUDA error";
     case ERF_ETOOLARGE: return "nx*ny*nz exceeds ERF_NOALLOC_MAX_VALUES, the fixed work space of erf_poisson_modes_noalloc";
@@ -117,6 +126,7 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
   c->gen_ready = false;
   c->graph_on = false;
   c->graph_warm = false;
+  c->graph_tick = 0;
   c->sc_Q = c->sc_Qt = c->sc_Qnew = c->sc_phi = c->sc_R = nullptr;
   c->sc_sum[0] = c->sc_sum[1] = c->sc_sum[2] = c->sc_G[0] = c->sc_G[1] = nullptr;
   c->an_pp = c->an_tw = c->an_lev = nullptr;
@@ -145,16 +155,16 @@ extern "C" int erf_create(const erf_grid *g, const erf_metrics *m, const erf_par
     c->base1d_r0 = c->alloc(g->nz);
     c->base1d_T0 = c->alloc(g->nz);
     if (!c->zl_dev || !c->base1d_r0 || !c->base1d_T0) { int rc = c->status; erf_destroy(c); return rc; }
-    cudaMemcpyAsync(c->zl_dev, m->z_levels, (g->nz + 1) * sizeof(double), cudaMemcpyHostToDevice, st);
-    cudaMemcpyAsync(c->base1d_r0, m->rho0, g->nz * sizeof(double), cudaMemcpyDeviceToDevice, st);
-    cudaMemcpyAsync(c->base1d_T0, m->rhotheta0, g->nz * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    copy(c, c->zl_dev, m->z_levels, (g->nz + 1) * sizeof(double), cudaMemcpyHostToDevice, st);
+    copy(c, c->base1d_r0, m->rho0, g->nz * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    copy(c, c->base1d_T0, m->rhotheta0, g->nz * sizeof(double), cudaMemcpyDeviceToDevice, st);
   } else {
     gen::NodeH Z;
     Z.zn = m->z_nodes; Z.zl = nullptr; Z.nx = g->nx; Z.ny = g->ny;
     if (!m->z_nodes) {
       c->zl_dev = c->alloc(g->nz + 1);
       if (!c->zl_dev) { int rc = c->status; erf_destroy(c); return rc; }
-      cudaMemcpyAsync(c->zl_dev, m->z_levels, (g->nz + 1) * sizeof(double), cudaMemcpyHostToDevice, st);
+      copy(c, c->zl_dev, m->z_levels, (g->nz + 1) * sizeof(double), cudaMemcpyHostToDevice, st);
       Z.zl = c->zl_dev;
     }
     int rc = build_general(c, Z, m->rho0, m->rhotheta0, m->base_is_1d, st);
@@ -178,11 +188,11 @@ extern "C" int erf_set_state(erf_ctx *c, const double *rho, const double *rhou, 
   if (c->status != ERF_OK) return c->status;
   cudaStream_t st = (cudaStream_t)stream;
   size_t nc = (size_t)c->nx * c->ny * c->nz * sizeof(double);
-  cudaMemcpyAsync(c->S.f[RHO], rho, nc, cudaMemcpyDeviceToDevice, st);
-  cudaMemcpyAsync(c->S.f[UU], rhou, nc, cudaMemcpyDeviceToDevice, st);
-  cudaMemcpyAsync(c->S.f[VV], rhov, nc, cudaMemcpyDeviceToDevice, st);
-  cudaMemcpyAsync(c->S.f[WW], rhow, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
-  cudaMemcpyAsync(c->S.f[TH], rhotheta, nc, cudaMemcpyDeviceToDevice, st);
+  copy(c, c->S.f[RHO], rho, nc, cudaMemcpyDeviceToDevice, st);
+  copy(c, c->S.f[UU], rhou, nc, cudaMemcpyDeviceToDevice, st);
+  copy(c, c->S.f[VV], rhov, nc, cudaMemcpyDeviceToDevice, st);
+  copy(c, c->S.f[WW], rhow, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  copy(c, c->S.f[TH], rhotheta, nc, cudaMemcpyDeviceToDevice, st);
   impose_lids(c, c->S, st);
   inflow_store(c, st);
   return check(c);
@@ -194,11 +204,11 @@ extern "C" int erf_get_state(erf_ctx *c, double *rho, double *rhou, double *rhov
   if (c->status != ERF_OK) return c->status;
   cudaStream_t st = (cudaStream_t)stream;
   size_t nc = (size_t)c->nx * c->ny * c->nz * sizeof(double);
-  if (rho) cudaMemcpyAsync(rho, c->S.f[RHO], nc, cudaMemcpyDeviceToDevice, st);
-  if (rhou) cudaMemcpyAsync(rhou, c->S.f[UU], nc, cudaMemcpyDeviceToDevice, st);
-  if (rhov) cudaMemcpyAsync(rhov, c->S.f[VV], nc, cudaMemcpyDeviceToDevice, st);
-  if (rhow) cudaMemcpyAsync(rhow, c->S.f[WW], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
-  if (rhotheta) cudaMemcpyAsync(rhotheta, c->S.f[TH], nc, cudaMemcpyDeviceToDevice, st);
+  if (rho) copy(c, rho, c->S.f[RHO], nc, cudaMemcpyDeviceToDevice, st);
+  if (rhou) copy(c, rhou, c->S.f[UU], nc, cudaMemcpyDeviceToDevice, st);
+  if (rhov) copy(c, rhov, c->S.f[VV], nc, cudaMemcpyDeviceToDevice, st);
+  if (rhow) copy(c, rhow, c->S.f[WW], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  if (rhotheta) copy(c, rhotheta, c->S.f[TH], nc, cudaMemcpyDeviceToDevice, st);
   return check(c);
 }
 
@@ -283,14 +293,14 @@ extern "C" int erf_set_scalar(erf_ctx *c, const double *rhophi, void *stream) {
   if (c->status != ERF_OK) return c->status;
   cudaStream_t st = (cudaStream_t)stream;
   if (ensure_general(c, st) != ERF_OK || !ensure_scalar(c)) return c->status;
-  cudaMemcpyAsync(c->sc_Q, rhophi, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  copy(c, c->sc_Q, rhophi, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice, st);
   return check(c);
 }
 
 extern "C" int erf_get_scalar(erf_ctx *c, double *rhophi, void *stream) {
   if (!c || !rhophi || !c->sc_Q) return ERF_EINVAL;
   if (c->status != ERF_OK) return c->status;
-  cudaMemcpyAsync(rhophi, c->sc_Q, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice,
+  copy(c, rhophi, c->sc_Q, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice,
                   (cudaStream_t)stream);
   return check(c);
 }
@@ -298,6 +308,7 @@ extern "C" int erf_get_scalar(erf_ctx *c, double *rhophi, void *stream) {
 extern "C" int erf_anelastic_step(erf_ctx *c, double dt, void *stream) {
   if (!c || !(dt > 0.0)) return ERF_EINVAL;
   if (c->status != ERF_OK) return c->status;
+  if (c->sc_Q) return ERF_EUNSUPPORTED;  // the RK2 step has no scalar stage: refuse rather than leave rho*phi frozen
   int rc = anelastic_step(c, dt, (cudaStream_t)stream);
   return rc != ERF_OK ? rc : check(c);
 }
@@ -312,7 +323,7 @@ extern "C" int erf_project(erf_ctx *c, double dt, void *stream) {
 extern "C" int erf_get_pprime(erf_ctx *c, double *pprime, void *stream) {
   if (!c || !pprime || !c->an_pp) return ERF_EINVAL;
   if (c->status != ERF_OK) return c->status;
-  cudaMemcpyAsync(pprime, c->an_pp, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice,
+  copy(c, pprime, c->an_pp, (size_t)c->nx * c->ny * c->nz * sizeof(double), cudaMemcpyDeviceToDevice,
                   (cudaStream_t)stream);
   return check(c);
 }
@@ -341,10 +352,39 @@ static void set_buffer_roles(erf_ctx *c, const std::vector<const void *> &r) {
   fused_set_buffer_roles(c, r, n);
 }
 
+// Graphs are kept for at most GRAPH_KEYS distinct (dt, n_acoustic) pairs; a caller whose dt changes from step to step
+// (a CFL-controlled step) would otherwise instantiate graphs without bound.  When a new pair arrives with the cache
+// full, every graph of the least recently used pair is destroyed (a graph still executing is released when it ends).
+constexpr int GRAPH_KEYS = 4;
+static void evict_graphs_for(erf_ctx *c, double dt, int ns) {
+  for (;;) {
+    std::vector<std::pair<double, int>> keys;
+    std::vector<long long> used;
+    for (auto &g : c->graphs) {
+      size_t n = 0;
+      while (n < keys.size() && !(keys[n].first == g.dt && keys[n].second == g.ns)) n++;
+      if (n == keys.size()) { keys.push_back({g.dt, g.ns}); used.push_back(g.last_use); }
+      else if (g.last_use > used[n]) used[n] = g.last_use;
+    }
+    bool present = false;
+    for (auto &k : keys) present |= k.first == dt && k.second == ns;
+    if (present || (int)keys.size() < GRAPH_KEYS) return;
+    size_t lru = 0;
+    for (size_t n = 1; n < keys.size(); n++)
+      if (used[n] < used[lru]) lru = n;
+    for (size_t n = c->graphs.size(); n-- > 0;)
+      if (c->graphs[n].dt == keys[lru].first && c->graphs[n].ns == keys[lru].second) {
+        cudaGraphExecDestroy(c->graphs[n].exec);
+        c->graphs.erase(c->graphs.begin() + n);
+      }
+  }
+}
+
 static int graph_step(erf_ctx *c, double dt, int ns, cudaStream_t st) {
   const std::vector<const void *> now = buffer_roles(c);
   for (auto &g : c->graphs)
     if (g.dt == dt && g.ns == ns && g.before == now) {
+      g.last_use = ++c->graph_tick;
       if (cudaGraphLaunch(g.exec, st) != cudaSuccess) c->status = ERF_ECUDA;
       set_buffer_roles(c, g.after);
       c->launches += g.launches;
@@ -355,8 +395,10 @@ static int graph_step(erf_ctx *c, double dt, int ns, cudaStream_t st) {
     fused_rk3_step(c, dt, ns, st);
     return check(c);
   }
+  evict_graphs_for(c, dt, ns);
   erf_ctx::StepGraph g;
   g.before = now; g.dt = dt; g.ns = ns;
+  g.last_use = ++c->graph_tick;
   const long long l0 = c->launches;
   cudaGraph_t graph = nullptr;
   if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
@@ -387,8 +429,8 @@ extern "C" int erf_rk3_step(erf_ctx *c, double dt, int n_acoustic, void *stream)
   }
   if (ensure_general(c, st) != ERF_OK) return c->status;
   for (int f = 0; f < 5; f++)  // S^t = S^n
-    cudaMemcpyAsync(c->St.f[f], c->S.f[f], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
-  if (c->sc_Q) cudaMemcpyAsync(c->sc_Qt, c->sc_Q, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+    copy(c, c->St.f[f], c->S.f[f], c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  if (c->sc_Q) copy(c, c->sc_Qt, c->sc_Q, c->NW * sizeof(double), cudaMemcpyDeviceToDevice, st);
   for (int stage = 1; stage <= 3; stage++) {
     int nsub; double dtau, dts;
     schedule(stage, dt, n_acoustic, &nsub, &dtau, &dts);
@@ -453,7 +495,7 @@ extern "C" int erf_slow_rhs(erf_ctx *c, double *R_rho, double *R_U, double *R_V,
   double *out[5] = {R_rho, R_U, R_V, R_W, R_Theta};
   for (int f = 0; f < 5; f++)
     if (out[f])
-      cudaMemcpyAsync(out[f], c->R.f[f], f == WW ? c->NW * sizeof(double) : nc, cudaMemcpyDeviceToDevice, st);
+      copy(c, out[f], c->R.f[f], f == WW ? c->NW * sizeof(double) : nc, cudaMemcpyDeviceToDevice, st);
   return check(c);
 }
 
@@ -475,13 +517,13 @@ extern "C" int erf_acoustic(erf_ctx *c, double dtau, int n, const double *R_rho,
   const double *Rin[5] = {R_rho, R_U, R_V, R_W, R_Theta};
   double *Pio[5] = {rho_pp, U_pp, V_pp, W_pp, Theta_pp};
   for (int f = 0; f < 5; f++) {
-    cudaMemcpyAsync(c->R.f[f], Rin[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
-    cudaMemcpyAsync(c->P.f[f], Pio[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
+    copy(c, c->R.f[f], Rin[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
+    copy(c, c->P.f[f], Pio[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
   }
   if (use_fused(c)) fused_acoustic(c, c->S, dtau, n, st);
   else if (c->path == ERF_PATH_AUTO && terrain_acoustic_available(c)) terrain_acoustic(c, c->S, dtau, n, st);
   else general_acoustic(c, c->S, dtau, n, st);
   for (int f = 0; f < 5; f++)
-    cudaMemcpyAsync(Pio[f], c->P.f[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
+    copy(c, Pio[f], c->P.f[f], f == WW ? nw : nc, cudaMemcpyDeviceToDevice, st);
   return check(c);
 }

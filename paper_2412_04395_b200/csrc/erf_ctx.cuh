@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <mutex>
 #include <vector>
 
 #include "../../include/erf_b200.h"
@@ -12,6 +13,23 @@ namespace erfb {
 
 struct F5 {
   double *f[5];
+};
+
+// Kernel function attributes (the opt-in to more than 48 KB of dynamic shared memory) belong to a device's context, not
+// to the process: a launch site keeps one OncePerDevice and sets its attributes the first time it runs on each GPU.
+struct OncePerDevice {
+  std::mutex mu;
+  unsigned long long seen = 0;
+  template <class F>
+  void run(F set_attributes) {
+    int dev = 0;
+    const bool known = cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < 64;
+    std::lock_guard<std::mutex> lock(mu);
+    const unsigned long long bit = known ? 1ull << dev : 0;
+    if (known && (seen & bit)) return;
+    set_attributes();  // an unknown device index: every time (correct, only slower)
+    seen |= bit;
+  }
 };
 
 struct FusedState;  // fused.cuh
@@ -66,10 +84,12 @@ struct erf_ctx {
     double dt;
     int ns;
     long long launches;
+    long long last_use;  // graph_tick at the last launch (least recently used (dt, n_acoustic) pair goes first)
     cudaGraphExec_t exec;
   };
   bool graph_on, graph_warm;  // warm: a plain step has run (kernel attributes are set outside any capture)
   std::vector<StepGraph> graphs;
+  long long graph_tick;
 
   // per-kernel timing (erf_set_timing)
   bool timing;

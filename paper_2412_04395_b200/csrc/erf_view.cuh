@@ -8,11 +8,7 @@
 #pragma once
 #include <cstddef>
 
-#ifdef __CUDACC__
-#define ERF_HD __host__ __device__ __forceinline__
-#else
-#define ERF_HD inline
-#endif
+#define ERF_HD __device__ __forceinline__  // every cell function runs on the device only
 
 namespace erfb {
 

@@ -34,6 +34,7 @@ constexpr int NW = 8;      // warps per CTA
 constexpr int CW = 32;     // columns per CTA
 
 __host__ __device__ constexpr size_t smem_bytes(int nz) { return ((size_t)3 * nz * CW + 2 * NW * CW) * sizeof(double); }
+constexpr size_t MAX_SMEM = 226 * 1024;  // dynamic shared memory the kernels opt in to
 
 // right-hand side of row k (S5): c1 = gamma Rd pi_f / hw, Bf = B_f(k), (.)_m = level k-1
 __device__ __forceinline__ double row_rhs(double om_b, double RW, double c1, double Bf, double That, double That_m,
@@ -286,7 +287,11 @@ __global__ void __launch_bounds__(32 * NW, 2) k_acoustic_tile(const AcArgs p, co
 template <int MODE>
 static void launch_mode(const AcArgs &p, dim3 grid, int chunk, size_t smem, cudaStream_t st) {
   void (*kern)(AcArgs, int) = p.write_cp ? k_acoustic_tile<MODE, true> : k_acoustic_tile<MODE, false>;
-  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  static OncePerDevice once;  // the opt-in covers every nz acoustic_tile_selected admits; the launch asks for what it uses
+  once.run([] {
+    cudaFuncSetAttribute(k_acoustic_tile<MODE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MAX_SMEM);
+    cudaFuncSetAttribute(k_acoustic_tile<MODE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MAX_SMEM);
+  });
   kern<<<grid, 32 * NW, smem, st>>>(p, chunk);
 }
 
@@ -302,7 +307,7 @@ static void launch_mode(const AcArgs &p, dim3 grid, int chunk, size_t smem, cuda
 // Developer knobs: ERF_VARIANT_FORCE_TILE / _FORCE_COLUMN.
 bool acoustic_tile_selected(const erf_ctx *c) {
   if (!c->fz || !c->fz->ok || (c->fz->variant & ERF_VARIANT_FORCE_COLUMN)) return false;
-  if (actile::smem_bytes(c->nz) > 226 * 1024) return false;  // 3 nz rows of 32 columns: nz <= 290
+  if (actile::smem_bytes(c->nz) > actile::MAX_SMEM) return false;  // 3 nz rows of 32 columns: nz <= 290
   if (c->fz->variant & ERF_VARIANT_FORCE_TILE) return true;
   return (long long)c->nx * c->ny <= 32768;
 }

@@ -276,8 +276,8 @@ int anelastic_project(erf_ctx *c, const F5 &S, double dt, cudaStream_t st) {
   const int lx = log2i(nx), ly = log2i(ny);  // -1: not a power of two, the direct sums run
   const size_t smfy = (size_t)(2 * 8 + 2) * ny * sizeof(double);
   const int tfx = nx / 2 < 256 ? (nx / 2 < 32 ? 32 : nx / 2) : 256;
-  static bool attr = false;
-  if (!attr) {
+  static OncePerDevice attr;
+  attr.run([] {
     cudaFuncSetAttribute(anel::k_fft_x<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(anel::k_fft_x<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(anel::k_fft_y<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -286,8 +286,7 @@ int anelastic_project(erf_ctx *c, const F5 &S, double dt, cudaStream_t st) {
     cudaFuncSetAttribute(anel::k_dft_x<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(anel::k_dft_y<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
     cudaFuncSetAttribute(anel::k_dft_y<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    attr = true;
-  }
+  });
   anel::k_div<<<grid, block, 0, st>>>(c->v, S.f[UU], S.f[VV], S.f[WW], c->an_lev, Br);
   const bool fy = ly > 0 && smfy <= 200 * 1024;
   dim3 gfy((nx + 7) / 8, nz);

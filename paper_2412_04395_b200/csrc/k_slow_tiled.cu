@@ -524,11 +524,8 @@ static int level_chunks(const erf_ctx *c, int *kchunk) {
 template <int OH, int FM>
 static void launch_adv_mask(const SlowFlat &p, dim3 grid, int kchunk, cudaStream_t st) {
   const size_t smem = NSTAGE * adv_stage(FM) * sizeof(double) + (ChunkSet<4, 3>::TAB + ChunkSet<2, 1>::TAB) * sizeof(int);
-  static bool once = false;
-  if (!once) {
-    cudaFuncSetAttribute(k_adv_tiled<OH, FM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    once = true;
-  }
+  static OncePerDevice once;
+  once.run([smem] { cudaFuncSetAttribute(k_adv_tiled<OH, FM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); });
   k_adv_tiled<OH, FM><<<grid, dim3(TX, TY), smem, st>>>(p, kchunk);
 }
 
@@ -581,11 +578,8 @@ void launch_visc_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st) {
   const int nch = level_chunks(c, &kchunk);
   dim3 grid((c->nx + TX - 1) / TX, (c->ny + TY - 1) / TY, nch);
   const size_t smem = VISC_NST * VISC_STAGE * sizeof(double) + ChunkSet<2, 1>::TAB * sizeof(int);
-  static bool once = false;
-  if (!once) {
-    cudaFuncSetAttribute(k_visc_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    once = true;
-  }
+  static OncePerDevice once;
+  once.run([smem] { cudaFuncSetAttribute(k_visc_tiled, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); });
   k_visc_tiled<<<grid, dim3(TX, TY), smem, st>>>(p, kchunk);
   c->launches++;
 }
@@ -593,11 +587,8 @@ void launch_visc_tiled(erf_ctx *c, const SlowFlat &p, cudaStream_t st) {
 template <int PART>
 static void launch_diff_part(const SlowFlat &p, dim3 grid, int kchunk, cudaStream_t st) {
   const size_t smem = NSTAGE * diff_stage(PART) * sizeof(double) + ChunkSet<2, 1>::TAB * sizeof(int);
-  static bool once = false;
-  if (!once) {
-    cudaFuncSetAttribute(k_diff_tiled<PART>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    once = true;
-  }
+  static OncePerDevice once;
+  once.run([smem] { cudaFuncSetAttribute(k_diff_tiled<PART>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); });
   k_diff_tiled<PART><<<grid, dim3(TX, TY), smem, st>>>(p, kchunk);
 }
 
