@@ -186,6 +186,17 @@ def median(xs):
     return xs[len(xs) // 2]
 
 
+def path_label(case):
+    """Which kernels erf_rk3_step picks for this case on ERF_PATH_AUTO (mirrors the library's host-side selection, so that
+    a fallback shows in the JSON line): k_slow_adv needs an even nx and nz + 1 <= 320, otherwise the round-1 slow-RHS
+    kernels run."""
+    if case.get("z_nodes") is not None:
+        return "terrain: fused advection + general diffusion passes + fused terrain substeps"
+    if case["nx"] % 2 == 0 and case["nz"] + 1 <= 320:
+        return "fused flat kernels"
+    return "fused flat kernels, round-1 slow RHS (k_slow_adv needs even nx and nz + 1 <= 320)"
+
+
 def time_config(binding, wl, torch, config, steps, warmup, repeats, graph, device):
     """One configuration, device-resident: median over `repeats` of the CUDA-event time of `steps` steps, the state
     reset before every repeat; on a side stream so that the CUDA-graph option can capture."""
@@ -219,7 +230,7 @@ def time_config(binding, wl, torch, config, steps, warmup, repeats, graph, devic
            "value": cells / (ms * 1e-3), "launches_per_step": launches, "launch": "cuda_graph" if graph else "stream",
            "algorithmic_bytes_per_cell": ad["total"] * 8,
            "whole_step_frac": ad["total"] * 8 * cells / (ms * 1e-3) / 1e9 / peak,
-           "path": "fused flat kernels" if case.get("z_nodes") is None else "terrain: fused advection + general diffusion passes + fused terrain substeps",
+           "path": path_label(case),
            "repeats": repeats, "steps": steps, "device_bytes": dyc.device_bytes}
     dyc.close()
     del dev
@@ -410,7 +421,7 @@ def run_ours(args):
 
     if roof is not None:
         # the fp64 FMA peak of this device, measured by the library's DFMA micro-benchmark; the fp64-pipe
-        # utilisation of each kernel against it is in profiles/r1_ncu_full_cfg5.md (ncu sm__pipe_fp64_cycles_active)
+        # utilisation of each kernel against it is in profiles/r2_ncu_full_cfg5.md (ncu sm__pipe_fp64_cycles_active)
         try:
             roof["fp64_peak_tflops"] = binding.erf_measure_fp64_peak()
         except Exception as e:  # pragma: no cover
@@ -433,7 +444,7 @@ def run_ours(args):
         all_cfg.append({"config": 5, "grid": f"{case['nx']}x{case['ny']}x{case['nz']}", "cells": cells,
                         "ms_per_step": ms / args.steps, "value": value, "launches_per_step": launches // args.steps,
                         "launch": "stream", "algorithmic_bytes_per_cell": ad["total"] * 8,
-                        "whole_step_frac": roof["whole_step"]["frac"] if roof else None, "path": "fused flat kernels",
+                        "whole_step_frac": roof["whole_step"]["frac"] if roof else None, "path": path_label(case),
                         "repeats": max(args.repeats, 1), "steps": args.steps})
 
     # ---- the oracle beside it, on a bounded sample (rank 0, N = 1 only)
