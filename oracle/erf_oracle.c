@@ -23,7 +23,16 @@
  * test_oracle_scalar.py (Eq. 4 with the averaged momenta), test_oracle_weno.py
  * (WENO-JS / WENO-Z from their definitions), test_oracle_open_rayleigh.py
  * (open and inflow boundaries, Rayleigh layer), test_oracle_anelastic.py
- * (Eq. 8, 14-16: dense brute-force projection, invariants, RK2 polynomial).
+ * (Eq. 8, 14-16: dense brute-force projection, invariants, RK2 polynomial);
+ * test_oracle_symmetry.py (round 3): slow_rhs, acoustic and a full step
+ * commute with the reflections of x and y and the exchange of x and y (flat
+ * and over an unsymmetric periodic terrain, orders 2-6) and, on a uniform
+ * column, with the reflection of z together with g -> -g: pins every two-
+ * and four-point mean and metric factor whose one-sided replacement is not
+ * symmetric (face density, face pi, edge viscosity, flux means, hu, hy, the
+ * metric pressure gradient).  Still unpinned: hw against hc in R_W over
+ * terrain, the size of omega in the substep, the chain-rule terms of the
+ * stress divergence (all symmetric under these maps).
  * The full nonlinear step on the benchmark configurations has no value
  * printed in the paper: "parity unpinned" beyond those invariants.
  *
