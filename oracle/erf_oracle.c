@@ -30,9 +30,11 @@
  * column, with the reflection of z together with g -> -g: pins every two-
  * and four-point mean and metric factor whose one-sided replacement is not
  * symmetric (face density, face pi, edge viscosity, flux means, hu, hy, the
- * metric pressure gradient).  Still unpinned: hw against hc in R_W over
- * terrain, the size of omega in the substep, the chain-rule terms of the
- * stress divergence (all symmetric under these maps).
+ * metric pressure gradient); test_oracle_appendix_a_terrain.py (round 3):
+ * the rho'' and Theta'' equations of a substep over terrain as residuals
+ * rebuilt with numpy from the node heights (pins the size and averaging of
+ * omega, hx / hy, the beta weights).  Still unpinned: hw against hc in R_W
+ * over terrain and the chain-rule terms of the stress divergence.
  * The full nonlinear step on the benchmark configurations has no value
  * printed in the paper: "parity unpinned" beyond those invariants.
  *
