@@ -404,12 +404,11 @@ bool slow_adv_available(const erf_ctx *c) { return (c->nx % 2) == 0 && c->nz + 1
 template <int OH, int OVT>
 static void launch_one(const SlowFlat &p, const sadv::Poly &poly, const sadv::Maps &maps, dim3 grid, int kchunk,
                        cudaStream_t st) {
-  static bool once = false;
-  if (!once) {
+  static OncePerDevice once;
+  once.run([] {
     cudaFuncSetAttribute(sadv::k_slow_adv<OH, OVT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                          (int)sadv::smem_bytes(sadv::MAXLEV));
-    once = true;
-  }
+  });
   sadv::k_slow_adv<OH, OVT><<<grid, sadv::NTH, sadv::smem_bytes(p.nz + 1), st>>>(p, poly, maps, kchunk);
 }
 
